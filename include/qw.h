@@ -1,0 +1,159 @@
+/* qw.h — C ABI of libqw: B200-native discrete-time coined quantum walk on Z^1 / Z^2.
+ *
+ * The library computes the repeated one-step evolution
+ *
+ *        psi(t+1) = U psi(t),      U = S (I (x) C)          (eq. 2; eq. 7)
+ *
+ * of Sawerwain & Gielerak, "GPGPU based simulations for one and two dimensional quantum walks"
+ * (arXiv 1003.3779): a local unitary coin C_v acts on every site's coin space (PAPER.md:35-38
+ * eq. 1), then the conditional shift S moves every coin component to its neighbour site
+ * (eq. 3; eq. 8), and finally the per-vertex probability
+ * distribution is formed by marginalising over the coin (Figs. 3-4).
+ * Every step of that path runs in hand-written CUDA kernels for sm_100a; there is no CPU
+ * fallback: every call returns QW_ECUDA when no device is usable.
+ *
+ * Conventions (DESIGN.md "Readings of the paper" lists each with its justification)
+ *   site index     1D: x in [0, extents[0]);  2D: m * extents[1] + n  (n fastest)
+ *   coin index     1D: 0 = R moves x -> x+1, 1 = L moves x -> x-1
+ *                  2D: c = 2j + k for the paper's |j,k>; QW_NATURAL lattice      (eq. 8)
+ *                        c0 -> (m, n+1)   c1 -> (m+1, n)   c2 -> (m-1, n)   c3 -> (m, n-1)
+ *                      QW_DIAGONAL lattice (Fig. 1c): (m + (-1)^j, n + (-1)^k)
+ *   one step       coin first, then shift
+ *   QW_PERIODIC    site indices taken modulo the extents
+ *   QW_OPEN        the links leaving the lattice are broken (RBL = 0 in PAPER.md:94-101,
+ *                  eqs. 9-10): the component stays on its site with the opposite coin
+ *                  (1D: 1-a; 2D: 3-c), no sign change.  U stays unitary.
+ *   complex        interleaved (re, im); QW_C128 = 2 x double, QW_C64 = 2 x float; coin
+ *                  matrices, phases and coin vectors use the dtype of the handle
+ *   user layout    "AoS": [batch][site][coin] complex.  The device layout (one plane per coin
+ *                  direction, PAPER-independent design choice) is private to the handle.
+ *
+ * Pointers: every data pointer (`const void *` / `void *` / `double *` / `uint8_t *`) may be a
+ * host pointer (pageable or pinned) or a device pointer; the library classifies it with
+ * cudaPointerGetAttributes.  Reading from / writing to host memory synchronises the handle's
+ * stream before the call returns; with device pointers the call is asynchronous on that
+ * stream.  `extents`, `site` and `qw_get_info`'s `out` are always host pointers.
+ *
+ * Ownership: the handle owns its device state (allocated by qw_create*, freed by qw_destroy).
+ * Callers own every buffer they pass; host buffers may be reused when the call returns,
+ * device buffers once the stream has passed the call.
+ *
+ * Errors: every call returns QW_OK (0) or a negative code, never throws or aborts; after an
+ * error the handle is unchanged (except QW_ECUDA raised by an asynchronous failure).
+ * qw_last_error() returns a thread-local message for the last non-zero return.
+ * A handle must not be used from two host threads at the same time.
+ */
+#ifndef QW_H_
+#define QW_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qw_sim qw_sim;
+
+enum { QW_OK = 0, QW_EINVAL = -1, QW_ENOMEM = -2, QW_ECUDA = -3, QW_ESTATE = -4, QW_EUNSUPPORTED = -5 };
+enum { QW_C64 = 0, QW_C128 = 1 };
+enum { QW_PERIODIC = 0, QW_OPEN = 1 };
+enum { QW_NATURAL = 0, QW_DIAGONAL = 1 };
+enum { QW_COIN_UNIFORM = 0, QW_COIN_PER_WALK = 1, QW_COIN_PER_SITE = 2 };
+
+/* Step schedules (qw_set_schedule).  All schedules compute bit-identical states. */
+enum {
+    QW_SCHED_AUTO = 0,     /* library picks: resident if a walk fits one CTA, else blocked / fused      */
+    QW_SCHED_GENERIC = 1,  /* one launch per step, one thread per site, every feature (reference kernel) */
+    QW_SCHED_FUSED = 2,    /* one launch per step, vectorised fused coin+shift (HBM-bound)              */
+    QW_SCHED_BLOCKED = 3,  /* temporally blocked: k steps per HBM round trip                            */
+    QW_SCHED_RESIDENT = 4  /* one CTA per walk, state on the SM for all n steps                         */
+};
+
+/* qw_get_info keys */
+enum {
+    QW_INFO_LAUNCHES = 0,       /* kernels launched by this handle so far                                */
+    QW_INFO_TIME = 1,           /* net number of steps applied since the last qw_set_state*              */
+    QW_INFO_LAST_SCHEDULE = 2,  /* schedule the last qw_step actually used (QW_SCHED_*)                   */
+    QW_INFO_LAST_K = 3,         /* temporal block depth of the last qw_step (1 if not blocked)           */
+    QW_INFO_STATE_BYTES = 4,    /* bytes of one device state buffer (there are two)                      */
+    QW_INFO_WINDOW = 5          /* 1 if the light-cone window is active                                  */
+};
+
+/* Create a walk on a dim-dimensional lattice (dim = 1 or 2) with `extents[d] >= 1` sites per
+ * axis.  coin_dim must equal 2*dim (degree of every vertex) else QW_EINVAL.
+ * qw_create == qw_create_batch(1, ...).  A batch holds `batch` independent walks on identical
+ * lattices (coin families may differ per walk and per vertex).
+ * On success *out is a new handle on the current CUDA device, stream 0, no coin, no state. */
+int qw_create(int dim, const int64_t *extents, int coin_dim, int dtype, int boundary, qw_sim **out);
+int qw_create_batch(int64_t batch, int dim, const int64_t *extents, int coin_dim, int dtype,
+                    int boundary, qw_sim **out);
+int qw_destroy(qw_sim *s);
+
+/* All later work of the handle is issued on `cuda_stream` (a cudaStream_t, e.g.
+ * torch.cuda.current_stream().cuda_stream; NULL = default stream). */
+int qw_set_stream(qw_sim *s, void *cuda_stream);
+
+/* 2D only: QW_NATURAL (default, eq. 8) or QW_DIAGONAL (Fig. 1c, the
+ * lattice of the paper's Tables 2-3). */
+int qw_set_lattice(qw_sim *s, int lattice);
+
+/* Coin family C = (C_v) (eq. 1).  `coin`: row-major coin_dim x coin_dim complex
+ * matrices, rows = output component: 1 matrix (UNIFORM), batch matrices (PER_WALK) or
+ * batch*sites matrices (PER_SITE, [walk][site]).  The library does not check unitarity. */
+int qw_set_coin(qw_sim *s, int mode, const void *coin);
+
+/* Optional unit-modulus multipliers [batch][site] applied on top of a UNIFORM / PER_WALK coin:
+ * C_{w,x} = phases[w][x] * C_w (BASELINE.json:configs[4]).  NULL removes them. */
+int qw_set_site_phases(qw_sim *s, const void *phases);
+
+/* Optional static broken links: mask[batch][site][coin] bytes, non-zero =
+ * the link that component `coin` of `site` would cross is broken; the component then stays on
+ * the site with the opposite coin (eq. 10 with RBL = 0).  Both ends of a link must carry the
+ * same bit (not checked).  NULL removes the mask. */
+int qw_set_broken_links(qw_sim *s, const uint8_t *mask);
+
+/* Set the state from AoS amplitudes [batch][site][coin]; resets the step counter.  The library
+ * never normalises (eq. 4 is the caller's responsibility). */
+int qw_set_state(qw_sim *s, const void *amps);
+
+/* Every walk of the batch: zero everywhere, `coin_vec` (coin_dim complex) at `site` (dim indices).
+ * Makes the light-cone window (eqs. 13-15, 17-18) available. */
+int qw_set_state_delta(qw_sim *s, const int64_t *site, const void *coin_vec);
+
+/* Copy the state out as AoS [batch][site][coin]. */
+int qw_get_state(const qw_sim *s, void *amps);
+
+/* n >= 0 applications of U (n = 0 is a no-op), asynchronous on the handle's stream.
+ * QW_ESTATE before qw_set_coin or qw_set_state*; QW_EINVAL for n < 0. */
+int qw_step(qw_sim *s, int64_t n);
+
+/* n applications of U^dagger = (I (x) C^dagger) S^dagger (reversibility checks). */
+int qw_step_inverse(qw_sim *s, int64_t n);
+
+/* P[w][x] = sum_a |psi[w][x][a]|^2: [batch][site] double (C128) / float (C64). */
+int qw_probabilities(const qw_sim *s, void *out);
+
+/* Per walk, in double regardless of dtype: 1D {norm, mean, var};
+ * 2D {norm, mean_m, mean_n, var_m, var_n, cov_mn}.  Coordinates x_d = index_d - floor(extent_d/2);
+ * mean and (population) variance are divided by the computed norm (eq. 4 fixes norm = 1). */
+int qw_moments(const qw_sim *s, double *out);
+
+/* Force a schedule (QW_SCHED_*); k = temporal block depth for QW_SCHED_BLOCKED (0 = library default).
+ * QW_EUNSUPPORTED if the handle's configuration has no such kernel. */
+int qw_set_schedule(qw_sim *s, int schedule, int k);
+
+/* Enable (1, default) / disable (0) the light-cone window: after qw_set_state_delta only sites
+ * within t+1 of the start are updated at step t.  Exact: skipped sites are 0. */
+int qw_set_window(qw_sim *s, int enable);
+
+int qw_get_info(const qw_sim *s, int what, int64_t *out);
+
+/* Block the host until the handle's stream is idle; reports asynchronous CUDA errors. */
+int qw_synchronize(const qw_sim *s);
+
+const char *qw_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QW_H_ */

@@ -1,0 +1,453 @@
+// qw_api.cu — the C ABI of include/qw.h: argument checking, device state ownership, host/device
+// pointer handling and the schedule dispatcher.  All arithmetic of the walk lives in the kernels
+// (qw_step*.cu, qw_reduce.cu); there is no CPU implementation of any step in this library.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "qw_internal.cuh"
+
+namespace qw {
+
+static thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+void clear_error() { g_err[0] = 0; }
+
+// true if p is device-accessible memory owned by the CUDA allocator (device or managed)
+static bool is_device_ptr(const void *p) {
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+static int ensure_scratch(qw_sim *s, size_t bytes) {
+    if (bytes <= s->scratch_bytes) return QW_OK;
+    if (s->scratch) { cudaStreamSynchronize(s->stream); cudaFree(s->scratch); s->scratch = nullptr; s->scratch_bytes = 0; }
+    cudaError_t e = cudaMalloc(&s->scratch, bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(QW_ENOMEM, "cannot allocate %zu bytes of staging memory", bytes); }
+    s->scratch_bytes = bytes;
+    return QW_OK;
+}
+
+static int classify_coin(const double *C, int cdim, int dtype) {
+    auto re = [&](int a, int b) { return C[2 * (a * cdim + b)]; };
+    auto im = [&](int a, int b) { return C[2 * (a * cdim + b) + 1]; };
+    bool real = true;
+    for (int i = 0; i < cdim * cdim; ++i) if (C[2 * i + 1] != 0.0) real = false;
+    if (cdim == 2) {
+        const double sv = re(0, 0);
+        if (real && sv != 0.0 && re(0, 1) == sv && re(1, 0) == sv && re(1, 1) == -sv) return COIN_HADAMARD;
+        return COIN_GENERAL;
+    }
+    const double h = re(0, 0);
+    if (real && h != 0.0) {
+        static const int sgn[4][4] = {{1, 1, 1, 1}, {1, -1, 1, -1}, {1, 1, -1, -1}, {1, -1, -1, 1}};
+        bool hxh = true;
+        for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) if (re(a, b) != sgn[a][b] * h) hxh = false;
+        if (hxh) return COIN_HXH4;
+    }
+    if (real) {
+        const double d = re(0, 0), g = re(0, 1);
+        bool gro = true;
+        for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) if (re(a, b) != (a == b ? d : g)) gro = false;
+        // the kernel evaluates g*sum + (d-g)*psi_a: only exact when d-g is representable
+        bool exact;
+        if (dtype == QW_C64) { volatile float dg = (float)d - (float)g; volatile float back = dg + (float)g; exact = (back == (float)d); }
+        else                 { volatile double dg = d - g; volatile double back = dg + g; exact = (back == d); }
+        if (gro && exact) return COIN_GROVER4;
+    }
+    if (h != 0.0 && im(0, 0) == 0.0) {
+        bool dft = true;
+        for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
+            const int p = (a * b) & 3;
+            const double wr = (p == 0) ? h : (p == 2 ? -h : 0.0);
+            const double wi = (p == 1) ? h : (p == 3 ? -h : 0.0);
+            if (re(a, b) != wr || im(a, b) != wi) dft = false;
+        }
+        if (dft) return COIN_DFT4;
+    }
+    return COIN_GENERAL;
+}
+
+// Source box of the next step (left = max(mid - extra - it, 1), ...).
+static Box step_box(const qw_sim *s) {
+    const Geom &g = s->g;
+    Box b{0, g.em - 1, 0, g.en - 1};
+    if (!s->window_enabled || !s->window_valid) return b;
+    const long long r = s->radius + 1;   // pad of one site, like the paper's `extra`
+    auto clampdim = [&](long long c, long long ext, long long &lo, long long &hi) {
+        long long l = c - r, h = c + r;
+        if (g.boundary == QW_PERIODIC) { if (l < 0 || h >= ext) { l = 0; h = ext - 1; } }
+        else { if (l < 0) l = 0; if (h >= ext) h = ext - 1; }
+        lo = l; hi = h;
+    };
+    if (g.dim == 1) clampdim(s->centre[0], g.en, b.n_lo, b.n_hi);
+    else { clampdim(s->centre[0], g.em, b.m_lo, b.m_hi); clampdim(s->centre[1], g.en, b.n_lo, b.n_hi); }
+    return b;
+}
+
+}  // namespace qw
+
+using namespace qw;
+
+extern "C" {
+
+const char *qw_last_error(void) { return g_err; }
+
+int qw_create_batch(int64_t batch, int dim, const int64_t *extents, int coin_dim, int dtype, int boundary,
+                    qw_sim **out) {
+    clear_error();
+    if (!out) return fail(QW_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!extents) return fail(QW_EINVAL, "extents is NULL");
+    if (dim != 1 && dim != 2) return fail(QW_EINVAL, "dim must be 1 or 2 (got %d)", dim);
+    if (coin_dim != 2 * dim) return fail(QW_EINVAL, "coin_dim must be 2*dim = %d (got %d)", 2 * dim, coin_dim);
+    if (dtype != QW_C64 && dtype != QW_C128) return fail(QW_EINVAL, "dtype must be QW_C64 or QW_C128");
+    if (boundary != QW_PERIODIC && boundary != QW_OPEN) return fail(QW_EINVAL, "boundary must be QW_PERIODIC or QW_OPEN");
+    if (batch < 1) return fail(QW_EINVAL, "batch must be >= 1");
+    for (int d = 0; d < dim; ++d)
+        if (extents[d] < 1) return fail(QW_EINVAL, "extents[%d] must be >= 1", d);
+
+    int dev = 0;
+    QW_CUDA(cudaGetDevice(&dev));
+    int sms = 0;
+    QW_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+
+    qw_sim *s = new (std::nothrow) qw_sim();
+    if (!s) return fail(QW_ENOMEM, "out of host memory");
+    memset(s, 0, sizeof(*s));
+    Geom &g = s->g;
+    g.dim = dim; g.cdim = coin_dim; g.boundary = boundary; g.lattice = QW_NATURAL;
+    g.batch = batch;
+    g.em = dim == 1 ? 1 : extents[0];
+    g.en = dim == 1 ? extents[0] : extents[1];
+    if (g.em > (1LL << 40) / g.en) { delete s; return fail(QW_EINVAL, "lattice too large"); }
+    g.sites = g.em * g.en;
+    s->dtype = dtype;
+    s->esize = dtype == QW_C128 ? 16 : 8;
+    // row pitch: 128-byte aligned rows when there is more than one row, else 16-byte aligned
+    const long long align_elems = ((batch * g.em > 1) ? 128 : 16) / (long long)s->esize;
+    g.pitch = (g.en + align_elems - 1) / align_elems * align_elems;
+    g.walk_stride = g.em * g.pitch;
+    g.plane_stride = g.batch * g.walk_stride;
+    s->device = dev; s->sm_count = sms; s->stream = 0;
+    s->state_bytes = (size_t)g.cdim * (size_t)g.plane_stride * s->esize;
+    s->window_enabled = true;
+    s->sched = QW_SCHED_AUTO; s->last_sched = QW_SCHED_AUTO; s->last_k = 1;
+    for (int i = 0; i < 2; ++i) {
+        cudaError_t e = cudaMalloc(&s->buf[i], s->state_bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            if (i == 1) cudaFree(s->buf[0]);
+            const size_t want = s->state_bytes;
+            delete s;
+            return fail(e == cudaErrorMemoryAllocation ? QW_ENOMEM : QW_ECUDA, "cudaMalloc(%zu) failed: %s",
+                        want, cudaGetErrorString(e));
+        }
+    }
+    cudaError_t e = cudaMemset(s->buf[0], 0, s->state_bytes);
+    if (e == cudaSuccess) e = cudaMemset(s->buf[1], 0, s->state_bytes);
+    if (e != cudaSuccess) {
+        cudaFree(s->buf[0]); cudaFree(s->buf[1]); delete s;
+        return fail(QW_ECUDA, "cudaMemset failed: %s", cudaGetErrorString(e));
+    }
+    *out = s;
+    return QW_OK;
+}
+
+int qw_create(int dim, const int64_t *extents, int coin_dim, int dtype, int boundary, qw_sim **out) {
+    return qw_create_batch(1, dim, extents, coin_dim, dtype, boundary, out);
+}
+
+int qw_destroy(qw_sim *s) {
+    clear_error();
+    if (!s) return QW_OK;
+    cudaStreamSynchronize(s->stream);
+    cudaFree(s->buf[0]); cudaFree(s->buf[1]);
+    if (s->d_coin) cudaFree(s->d_coin);
+    if (s->d_phases) cudaFree(s->d_phases);
+    if (s->d_broken) cudaFree(s->d_broken);
+    if (s->scratch) cudaFree(s->scratch);
+    if (s->partials) cudaFree(s->partials);
+    cudaGetLastError();
+    delete s;
+    return QW_OK;
+}
+
+int qw_set_stream(qw_sim *s, void *cuda_stream) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_CUDA(cudaStreamSynchronize(s->stream));   // keep work already issued ordered before the switch
+    s->stream = static_cast<cudaStream_t>(cuda_stream);
+    return QW_OK;
+}
+
+int qw_set_lattice(qw_sim *s, int lattice) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (lattice != QW_NATURAL && lattice != QW_DIAGONAL) return fail(QW_EINVAL, "unknown lattice kind %d", lattice);
+    if (s->g.dim == 1 && lattice == QW_DIAGONAL) return fail(QW_EINVAL, "the diagonal lattice is 2D only");
+    s->g.lattice = lattice;
+    return QW_OK;
+}
+
+int qw_set_coin(qw_sim *s, int mode, const void *coin) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (!coin) return fail(QW_EINVAL, "coin is NULL");
+    if (mode != QW_COIN_UNIFORM && mode != QW_COIN_PER_WALK && mode != QW_COIN_PER_SITE)
+        return fail(QW_EINVAL, "unknown coin mode %d", mode);
+    const Geom &g = s->g;
+    const size_t one = (size_t)g.cdim * g.cdim * s->esize;
+    if (mode == QW_COIN_UNIFORM) {
+        unsigned char tmp[16 * 16];
+        if (is_device_ptr(coin)) {
+            QW_CUDA(cudaMemcpyAsync(tmp, coin, one, cudaMemcpyDeviceToHost, s->stream));
+            QW_CUDA(cudaStreamSynchronize(s->stream));
+        } else {
+            memcpy(tmp, coin, one);
+        }
+        for (int i = 0; i < 2 * g.cdim * g.cdim; ++i)
+            s->h_coin[i] = s->dtype == QW_C128 ? reinterpret_cast<double *>(tmp)[i] : (double)reinterpret_cast<float *>(tmp)[i];
+        s->coin_kind = classify_coin(s->h_coin, g.cdim, s->dtype);
+        if (s->d_coin) { QW_CUDA(cudaStreamSynchronize(s->stream)); cudaFree(s->d_coin); s->d_coin = nullptr; }
+    } else {
+        const size_t count = mode == QW_COIN_PER_WALK ? (size_t)g.batch : (size_t)g.batch * (size_t)g.sites;
+        void *d = nullptr;
+        cudaError_t e = cudaMalloc(&d, count * one);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(QW_ENOMEM, "cannot allocate %zu bytes for the coin family", count * one); }
+        cudaError_t e2 = cudaMemcpyAsync(d, coin, count * one, is_device_ptr(coin) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream);
+        if (e2 != cudaSuccess) { cudaFree(d); return fail(QW_ECUDA, "copy of the coin family failed: %s", cudaGetErrorString(e2)); }
+        QW_CUDA(cudaStreamSynchronize(s->stream));
+        if (s->d_coin) cudaFree(s->d_coin);
+        s->d_coin = d;
+        s->coin_kind = COIN_GENERAL;
+    }
+    s->coin_mode = mode;
+    s->has_coin = true;
+    return QW_OK;
+}
+
+int qw_set_site_phases(qw_sim *s, const void *phases) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    if (!phases) { if (s->d_phases) cudaFree(s->d_phases); s->d_phases = nullptr; return QW_OK; }
+    const size_t bytes = (size_t)s->g.batch * (size_t)s->g.sites * s->esize;
+    void *d = nullptr;
+    if (cudaMalloc(&d, bytes) != cudaSuccess) { cudaGetLastError(); return fail(QW_ENOMEM, "cannot allocate %zu bytes for the phases", bytes); }
+    cudaError_t e = cudaMemcpyAsync(d, phases, bytes, is_device_ptr(phases) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream);
+    if (e != cudaSuccess) { cudaFree(d); return fail(QW_ECUDA, "copy of the phases failed: %s", cudaGetErrorString(e)); }
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    if (s->d_phases) cudaFree(s->d_phases);
+    s->d_phases = d;
+    return QW_OK;
+}
+
+int qw_set_broken_links(qw_sim *s, const uint8_t *mask) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    if (!mask) { if (s->d_broken) cudaFree(s->d_broken); s->d_broken = nullptr; return QW_OK; }
+    const size_t bytes = (size_t)s->g.batch * (size_t)s->g.sites * (size_t)s->g.cdim;
+    void *d = nullptr;
+    if (cudaMalloc(&d, bytes) != cudaSuccess) { cudaGetLastError(); return fail(QW_ENOMEM, "cannot allocate %zu bytes for the link mask", bytes); }
+    cudaError_t e = cudaMemcpyAsync(d, mask, bytes, is_device_ptr(mask) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->stream);
+    if (e != cudaSuccess) { cudaFree(d); return fail(QW_ECUDA, "copy of the link mask failed: %s", cudaGetErrorString(e)); }
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    if (s->d_broken) cudaFree(s->d_broken);
+    s->d_broken = static_cast<uint8_t *>(d);
+    return QW_OK;
+}
+
+int qw_set_state(qw_sim *s, const void *amps) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (!amps) return fail(QW_EINVAL, "amps is NULL");
+    const Geom &g = s->g;
+    const size_t bytes = (size_t)g.batch * (size_t)g.sites * (size_t)g.cdim * s->esize;
+    const void *src = amps;
+    if (!is_device_ptr(amps)) {
+        int rc = ensure_scratch(s, bytes);
+        if (rc) return rc;
+        QW_CUDA(cudaMemcpyAsync(s->scratch, amps, bytes, cudaMemcpyHostToDevice, s->stream));
+        src = s->scratch;
+    }
+    s->cur = 0;
+    if (g.pitch != g.en) QW_CUDA(cudaMemsetAsync(s->buf[0], 0, s->state_bytes, s->stream));
+    int rc = launch_aos_to_soa(s, src, s->buf[0]);
+    if (rc) return rc;
+    if (src == s->scratch) QW_CUDA(cudaStreamSynchronize(s->stream));   // host buffer reusable on return
+    s->has_state = true; s->t = 0; s->window_valid = false;
+    return QW_OK;
+}
+
+int qw_set_state_delta(qw_sim *s, const int64_t *site, const void *coin_vec) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (!site || !coin_vec) return fail(QW_EINVAL, "site or coin_vec is NULL");
+    const Geom &g = s->g;
+    long long st[2] = {0, 0};
+    for (int d = 0; d < g.dim; ++d) {
+        const long long ext = (g.dim == 1) ? g.en : (d == 0 ? g.em : g.en);
+        if (site[d] < 0 || site[d] >= ext) return fail(QW_EINVAL, "site[%d] = %lld outside [0, %lld)", d, (long long)site[d], ext);
+        st[d] = site[d];
+    }
+    unsigned char tmp[64];
+    const size_t vb = (size_t)g.cdim * s->esize;
+    if (is_device_ptr(coin_vec)) {
+        QW_CUDA(cudaMemcpyAsync(tmp, coin_vec, vb, cudaMemcpyDeviceToHost, s->stream));
+        QW_CUDA(cudaStreamSynchronize(s->stream));
+    } else {
+        memcpy(tmp, coin_vec, vb);
+    }
+    double cv[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (int i = 0; i < 2 * g.cdim; ++i)
+        cv[i] = s->dtype == QW_C128 ? reinterpret_cast<double *>(tmp)[i] : (double)reinterpret_cast<float *>(tmp)[i];
+    QW_CUDA(cudaMemsetAsync(s->buf[0], 0, s->state_bytes, s->stream));
+    QW_CUDA(cudaMemsetAsync(s->buf[1], 0, s->state_bytes, s->stream));
+    s->cur = 0;
+    int rc = launch_delta(s, st, cv);
+    if (rc) return rc;
+    s->has_state = true; s->t = 0;
+    s->window_valid = true; s->radius = 0;
+    s->centre[0] = st[0]; s->centre[1] = st[1];
+    return QW_OK;
+}
+
+int qw_get_state(const qw_sim *cs, void *amps) {
+    clear_error();
+    qw_sim *s = const_cast<qw_sim *>(cs);
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (!amps) return fail(QW_EINVAL, "amps is NULL");
+    if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
+    const Geom &g = s->g;
+    const size_t bytes = (size_t)g.batch * (size_t)g.sites * (size_t)g.cdim * s->esize;
+    if (is_device_ptr(amps)) return launch_soa_to_aos(s, s->buf[s->cur], amps);
+    int rc = ensure_scratch(s, bytes);
+    if (rc) return rc;
+    rc = launch_soa_to_aos(s, s->buf[s->cur], s->scratch);
+    if (rc) return rc;
+    QW_CUDA(cudaMemcpyAsync(amps, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    return QW_OK;
+}
+
+int qw_step(qw_sim *s, int64_t n) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (n < 0) return fail(QW_EINVAL, "n must be >= 0 (got %lld)", (long long)n);
+    if (!s->has_coin) return fail(QW_ESTATE, "qw_step before qw_set_coin");
+    if (!s->has_state) return fail(QW_ESTATE, "qw_step before qw_set_state");
+    if (n == 0) return QW_OK;
+    const bool allow_fast = s->sched != QW_SCHED_GENERIC;
+    s->last_sched = allow_fast ? QW_SCHED_FUSED : QW_SCHED_GENERIC;
+    s->last_k = 1;
+    for (int64_t i = 0; i < n; ++i) {
+        const Box box = step_box(s);
+        int rc = launch_step(s, s->buf[s->cur], s->buf[1 - s->cur], box, allow_fast);
+        if (rc) return rc;
+        s->cur ^= 1; s->t += 1; s->radius += 1;
+    }
+    return QW_OK;
+}
+
+int qw_step_inverse(qw_sim *s, int64_t n) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (n < 0) return fail(QW_EINVAL, "n must be >= 0 (got %lld)", (long long)n);
+    if (!s->has_coin) return fail(QW_ESTATE, "qw_step_inverse before qw_set_coin");
+    if (!s->has_state) return fail(QW_ESTATE, "qw_step_inverse before qw_set_state");
+    for (int64_t i = 0; i < n; ++i) {
+        int rc = launch_step_inverse(s, s->buf[s->cur], s->buf[1 - s->cur]);
+        if (rc) return rc;
+        s->cur ^= 1; s->t -= 1; s->radius += 1;
+    }
+    return QW_OK;
+}
+
+int qw_probabilities(const qw_sim *cs, void *out) {
+    clear_error();
+    qw_sim *s = const_cast<qw_sim *>(cs);
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (!out) return fail(QW_EINVAL, "out is NULL");
+    if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
+    const size_t bytes = (size_t)s->g.batch * (size_t)s->g.sites * (s->esize / 2);
+    if (is_device_ptr(out)) return launch_probabilities(s, s->buf[s->cur], out);
+    int rc = ensure_scratch(s, bytes);
+    if (rc) return rc;
+    rc = launch_probabilities(s, s->buf[s->cur], s->scratch);
+    if (rc) return rc;
+    QW_CUDA(cudaMemcpyAsync(out, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    return QW_OK;
+}
+
+int qw_moments(const qw_sim *cs, double *out) {
+    clear_error();
+    qw_sim *s = const_cast<qw_sim *>(cs);
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (!out) return fail(QW_EINVAL, "out is NULL");
+    if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
+    const size_t bytes = (size_t)s->g.batch * (s->g.dim == 1 ? 3 : 6) * sizeof(double);
+    if (is_device_ptr(out)) return launch_moments(s, s->buf[s->cur], out);
+    int rc = ensure_scratch(s, bytes);
+    if (rc) return rc;
+    rc = launch_moments(s, s->buf[s->cur], static_cast<double *>(s->scratch));
+    if (rc) return rc;
+    QW_CUDA(cudaMemcpyAsync(out, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    return QW_OK;
+}
+
+int qw_set_schedule(qw_sim *s, int schedule, int k) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (schedule < QW_SCHED_AUTO || schedule > QW_SCHED_RESIDENT) return fail(QW_EINVAL, "unknown schedule %d", schedule);
+    if (k < 0) return fail(QW_EINVAL, "k must be >= 0");
+    if (schedule == QW_SCHED_BLOCKED || schedule == QW_SCHED_RESIDENT)
+        return fail(QW_EUNSUPPORTED, "schedule %d is not available for this configuration", schedule);
+    s->sched = schedule; s->sched_k = k;
+    return QW_OK;
+}
+
+int qw_set_window(qw_sim *s, int enable) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    s->window_enabled = enable != 0;
+    return QW_OK;
+}
+
+int qw_get_info(const qw_sim *s, int what, int64_t *out) {
+    clear_error();
+    if (!s || !out) return fail(QW_EINVAL, "NULL argument");
+    switch (what) {
+        case QW_INFO_LAUNCHES: *out = s->launches; break;
+        case QW_INFO_TIME: *out = s->t; break;
+        case QW_INFO_LAST_SCHEDULE: *out = s->last_sched; break;
+        case QW_INFO_LAST_K: *out = s->last_k; break;
+        case QW_INFO_STATE_BYTES: *out = (int64_t)s->state_bytes; break;
+        case QW_INFO_WINDOW: *out = (s->window_enabled && s->window_valid) ? 1 : 0; break;
+        default: return fail(QW_EINVAL, "unknown info key %d", what);
+    }
+    return QW_OK;
+}
+
+int qw_synchronize(const qw_sim *s) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    return QW_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,148 @@
+// qw_coin.cuh — the per-site coin arithmetic phi = C psi (eq. 1; the inner sum of
+// PAPER.md:101 eq. 10), shared by EVERY step kernel of the library so that all schedules
+// (generic, fused, temporally blocked, resident) execute the same instruction sequence per site
+// and therefore produce bit-identical states.  Every operation is an explicit round-to-nearest
+// intrinsic: the compiler may neither contract nor re-associate them.
+#pragma once
+
+#include "qw_internal.cuh"
+
+namespace qw {
+
+__device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ float  fma_rn(float a, float b, float c)    { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float  mul_rn(float a, float b)   { return __fmul_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float  add_rn(float a, float b)   { return __fadd_rn(a, b); }
+__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ float  sub_rn(float a, float b)   { return __fsub_rn(a, b); }
+
+template <typename R> struct cplx { R re, im; };
+
+template <typename R> __device__ __forceinline__ cplx<R> cx_load(const typename Cx<R>::T *p) {
+    typename Cx<R>::T v = *p;
+    return cplx<R>{v.x, v.y};
+}
+template <typename R> __device__ __forceinline__ void cx_store(typename Cx<R>::T *p, cplx<R> z) {
+    typename Cx<R>::T v; v.x = z.re; v.y = z.im;
+    *p = v;
+}
+
+// c * z
+template <typename R> __device__ __forceinline__ cplx<R> cx_mul(R cre, R cim, cplx<R> z) {
+    cplx<R> r;
+    r.re = fma_rn(-cim, z.im, mul_rn(cre, z.re));
+    r.im = fma_rn(cim, z.re, mul_rn(cre, z.im));
+    return r;
+}
+// acc + c * z
+template <typename R> __device__ __forceinline__ cplx<R> cx_fma(R cre, R cim, cplx<R> z, cplx<R> acc) {
+    acc.re = fma_rn(cre, z.re, acc.re);
+    acc.re = fma_rn(-cim, z.im, acc.re);
+    acc.im = fma_rn(cre, z.im, acc.im);
+    acc.im = fma_rn(cim, z.re, acc.im);
+    return acc;
+}
+template <typename R> __device__ __forceinline__ cplx<R> cx_add(cplx<R> a, cplx<R> b) {
+    return cplx<R>{add_rn(a.re, b.re), add_rn(a.im, b.im)};
+}
+template <typename R> __device__ __forceinline__ cplx<R> cx_sub(cplx<R> a, cplx<R> b) {
+    return cplx<R>{sub_rn(a.re, b.re), sub_rn(a.im, b.im)};
+}
+template <typename R> __device__ __forceinline__ cplx<R> cx_scale(R s, cplx<R> a) {
+    return cplx<R>{mul_rn(s, a.re), mul_rn(s, a.im)};
+}
+// i * a,  -i * a   (exact)
+template <typename R> __device__ __forceinline__ cplx<R> cx_muli(cplx<R> a)  { return cplx<R>{-a.im, a.re}; }
+template <typename R> __device__ __forceinline__ cplx<R> cx_mulni(cplx<R> a) { return cplx<R>{a.im, -a.re}; }
+
+// phi = C psi in place.  C: row-major CD x CD complex, interleaved (re, im), rows = output component.
+// KIND selects an algebraically equal, cheaper evaluation for the named coins of PAPER.md:82
+// (Hadamard, Grover, Fourier) — the host classifies the matrix (qw_api.cu: classify_coin) and only
+// picks a special kind when the matrix entries match that pattern exactly.
+template <typename R, int CD, int KIND>
+__device__ __forceinline__ void apply_coin(const R *__restrict__ C, cplx<R> (&v)[CD]) {
+    if constexpr (KIND == COIN_HADAMARD && CD == 2) {
+        // s*[[1,1],[1,-1]]: 4 add/sub + 4 mul
+        const R s = C[0];
+        cplx<R> p = cx_add(v[0], v[1]);
+        cplx<R> m = cx_sub(v[0], v[1]);
+        v[0] = cx_scale(s, p);
+        v[1] = cx_scale(s, m);
+    } else if constexpr (KIND == COIN_GROVER4 && CD == 4) {
+        // off-diagonal g, diagonal d (Grover: g = 1/2, d = -1/2): phi_a = g*sum + (d-g)*psi_a
+        const R g = C[2], dg = sub_rn(C[0], C[2]);
+        cplx<R> sum = cx_add(cx_add(v[0], v[1]), cx_add(v[2], v[3]));
+        cplx<R> gs = cx_scale(g, sum);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            v[a].re = fma_rn(dg, v[a].re, gs.re);
+            v[a].im = fma_rn(dg, v[a].im, gs.im);
+        }
+    } else if constexpr (KIND == COIN_HXH4 && CD == 4) {
+        // h * (H (x) H) with c = 2j+k: butterfly over k, then over j, then one scale
+        const R h = C[0];
+        cplx<R> a0 = cx_add(v[0], v[1]), a1 = cx_sub(v[0], v[1]);
+        cplx<R> a2 = cx_add(v[2], v[3]), a3 = cx_sub(v[2], v[3]);
+        v[0] = cx_scale(h, cx_add(a0, a2));
+        v[1] = cx_scale(h, cx_add(a1, a3));
+        v[2] = cx_scale(h, cx_sub(a0, a2));
+        v[3] = cx_scale(h, cx_sub(a1, a3));
+    } else if constexpr (KIND == COIN_DFT4 && CD == 4) {
+        // h * i^(ab): radix-2 decimation: e = v0 +- v2, o = v1 +- v3
+        const R h = C[0];
+        cplx<R> e0 = cx_add(v[0], v[2]), e1 = cx_sub(v[0], v[2]);
+        cplx<R> o0 = cx_add(v[1], v[3]), o1 = cx_muli(cx_sub(v[1], v[3]));
+        v[0] = cx_scale(h, cx_add(e0, o0));
+        v[1] = cx_scale(h, cx_add(e1, o1));
+        v[2] = cx_scale(h, cx_sub(e0, o0));
+        v[3] = cx_scale(h, cx_sub(e1, o1));
+    } else {
+        cplx<R> out[CD];
+#pragma unroll
+        for (int a = 0; a < CD; ++a) {
+            cplx<R> acc = cx_mul(C[2 * (a * CD) + 0], C[2 * (a * CD) + 1], v[0]);
+#pragma unroll
+            for (int b = 1; b < CD; ++b)
+                acc = cx_fma(C[2 * (a * CD + b) + 0], C[2 * (a * CD + b) + 1], v[b], acc);
+            out[a] = acc;
+        }
+#pragma unroll
+        for (int a = 0; a < CD; ++a) v[a] = out[a];
+    }
+}
+
+// psi = C^dagger phi in place (inverse step; general evaluation only).
+template <typename R, int CD>
+__device__ __forceinline__ void apply_coin_dagger(const R *__restrict__ C, cplx<R> (&v)[CD]) {
+    cplx<R> out[CD];
+#pragma unroll
+    for (int b = 0; b < CD; ++b) {
+        cplx<R> acc = cx_mul(C[2 * (0 * CD + b) + 0], -C[2 * (0 * CD + b) + 1], v[0]);
+#pragma unroll
+        for (int a = 1; a < CD; ++a)
+            acc = cx_fma(C[2 * (a * CD + b) + 0], -C[2 * (a * CD + b) + 1], v[a], acc);
+        out[b] = acc;
+    }
+#pragma unroll
+    for (int b = 0; b < CD; ++b) v[b] = out[b];
+}
+
+// Direction of coin component `a`: (dm, dn).  1D uses dn only.
+template <int DIM>
+__device__ __forceinline__ void coin_direction(int lattice, int a, int &dm, int &dn) {
+    if constexpr (DIM == 1) {
+        dm = 0; dn = (a == 0) ? +1 : -1;                    // R: x+1, L: x-1
+    } else {
+        if (lattice == QW_NATURAL) {                        // PAPER.md:88 eq. 8, c = 2j+k
+            dm = (a == 1) ? +1 : (a == 2 ? -1 : 0);
+            dn = (a == 0) ? +1 : (a == 3 ? -1 : 0);
+        } else {                                            // PAPER.md:106 Fig. 1c: (m+(-1)^j, n+(-1)^k)
+            dm = (a & 2) ? -1 : +1;
+            dn = (a & 1) ? -1 : +1;
+        }
+    }
+}
+
+}  // namespace qw

@@ -1,0 +1,125 @@
+// qw_internal.cuh — private declarations shared by the translation units of libqw.
+// Nothing here is part of the C ABI (include/qw.h) and nothing is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/qw.h"
+
+namespace qw {
+
+// ---------------------------------------------------------------------------------------------
+// Device layout: structure of arrays, one contiguous complex
+// plane per coin direction:  plane[c][walk][m][n_pitch].  Two such buffers (ping-pong).
+// ---------------------------------------------------------------------------------------------
+struct Geom {
+    int dim;          // 1 or 2
+    int cdim;         // 2 * dim
+    int boundary;     // QW_PERIODIC / QW_OPEN
+    int lattice;      // QW_NATURAL / QW_DIAGONAL
+    long long batch;
+    long long em, en;        // 1D: em = 1, en = extent
+    long long sites;         // em * en
+    long long pitch;         // complex elements per lattice row (>= en, padded)
+    long long walk_stride;   // em * pitch
+    long long plane_stride;  // batch * walk_stride
+};
+
+enum CoinKind {
+    COIN_GENERAL = 0,   // full complex mat-vec
+    COIN_HADAMARD = 1,  // 1D: s*[[1,1],[1,-1]], s real
+    COIN_GROVER4 = 2,   // 2D: g*J - I-like: off-diagonal all equal real g, diagonal g-1... see qw_coin.cuh
+    COIN_HXH4 = 3,      // 2D: h*[[1,1,1,1],[1,-1,1,-1],[1,1,-1,-1],[1,-1,-1,1]], h real
+    COIN_DFT4 = 4       // 2D: h*i^(ab), h real
+};
+
+template <typename R> struct Cx;
+template <> struct Cx<double> { typedef double2 T; };
+template <> struct Cx<float>  { typedef float2 T; };
+
+// Source-site box updated by one step (light-cone window).  Inclusive bounds.
+struct Box { long long m_lo, m_hi, n_lo, n_hi; };
+
+}  // namespace qw
+
+// The opaque handle of include/qw.h.
+struct qw_sim {
+    qw::Geom g;
+    int dtype;               // QW_C64 / QW_C128
+    size_t esize;            // bytes per complex amplitude
+    int device;
+    int sm_count;
+    cudaStream_t stream;
+
+    void *buf[2];            // ping-pong state buffers, each cdim * plane_stride complex
+    int cur;                 // buf[cur] holds psi(t)
+    size_t state_bytes;
+
+    // coin family
+    bool has_coin;
+    int coin_mode;
+    int coin_kind;           // qw::CoinKind, classified from the uniform matrix
+    double h_coin[32];       // uniform coin, complex interleaved, promoted to double
+    void *d_coin;            // PER_WALK / PER_SITE matrices on the device (handle dtype)
+    void *d_phases;          // optional [batch][site] complex multipliers
+    uint8_t *d_broken;       // optional [batch][site][coin] link mask
+
+    // state bookkeeping
+    bool has_state;
+    long long t;             // net steps since set_state
+    bool window_enabled;     // user switch
+    bool window_valid;       // both buffers are zero outside the box below
+    long long centre[2];
+    long long radius;        // support of psi(t) is within `radius` of `centre` (Chebyshev)
+
+    // schedule
+    int sched, sched_k;
+    int last_sched, last_k;
+    long long launches;
+
+    // scratch
+    void *scratch;           // staging for host <-> device transposes and outputs
+    size_t scratch_bytes;
+    double *partials;        // moment partial sums
+    size_t partials_count;
+};
+
+namespace qw {
+
+// error reporting (qw_api.cu)
+int fail(int code, const char *fmt, ...);
+void clear_error();
+
+#define QW_CUDA(call)                                                                         \
+    do {                                                                                      \
+        cudaError_t qw_e_ = (call);                                                           \
+        if (qw_e_ != cudaSuccess)                                                             \
+            return ::qw::fail(QW_ECUDA, "%s failed: %s", #call, cudaGetErrorString(qw_e_));   \
+    } while (0)
+
+#define QW_LAUNCH_CHECK(s, name)                                                              \
+    do {                                                                                      \
+        cudaError_t qw_e_ = cudaGetLastError();                                               \
+        if (qw_e_ != cudaSuccess)                                                             \
+            return ::qw::fail(QW_ECUDA, "launch of %s failed: %s", name,                      \
+                              cudaGetErrorString(qw_e_));                                     \
+        (s)->launches++;                                                                      \
+    } while (0)
+
+// ---- kernels' host-side launchers (one per translation unit) -------------------------------
+// qw_layout.cu
+int launch_aos_to_soa(qw_sim *s, const void *aos_dev, void *soa);
+int launch_soa_to_aos(qw_sim *s, const void *soa, void *aos_dev);
+int launch_delta(qw_sim *s, const long long *site, const double *coin_vec);
+
+// qw_step.cu : one launch per step, scatter form.  fast = uniform coin, no phases, no links, natural.
+int launch_step(qw_sim *s, const void *in, void *out, const Box &box, bool allow_fast);
+int launch_step_inverse(qw_sim *s, const void *in, void *out);
+
+// qw_reduce.cu
+int launch_probabilities(qw_sim *s, const void *state, void *out_dev);
+int launch_moments(qw_sim *s, const void *state, double *out_dev);
+
+}  // namespace qw

@@ -1,0 +1,250 @@
+// qw_step.cu — one-launch-per-step kernels: the fused coin + conditional-shift step
+// psi' = S (I (x) C) psi (PAPER.md:42 eq. 2, :80 eq. 7) in SCATTER form: the thread that owns
+// source site x applies the coin in registers (eq. 1) and writes every component straight into
+// its neighbour site of the other ping-pong buffer (eq. 3 / eq. 8); components whose link is
+// broken or leaves an open lattice are written back to x with the opposite coin (eqs. 9-10).
+// Each amplitude is read once and written once: 2 * coin_dim * sizeof(complex) bytes per site.
+//
+// Two instantiation families share the code:
+//   FAST    uniform coin held in the kernel parameters (constant bank), no phases, no link
+//           mask, natural lattice; U sites per thread, strided by the block so that every warp
+//           access is one contiguous run                       -> QW_SCHED_FUSED
+//   GENERAL every feature decided at run time (per-walk / per-site coins, phases, broken links,
+//           diagonal lattice)                                  -> QW_SCHED_GENERIC
+// plus the inverse step U^dagger in gather form (qw_step_inverse).
+#include "qw_coin.cuh"
+
+namespace qw {
+
+template <typename R, int CD>
+struct StepArgs {
+    const typename Cx<R>::T *in;
+    typename Cx<R>::T *out;
+    long long em, en, pitch, walk_stride, plane_stride, sites;
+    long long m_lo, n_lo;        // origin of the source box
+    long long box_m, box_n;      // extent of the source box
+    int chunks_per_row;          // blocks along n
+    int boundary, lattice, coin_mode;
+    const typename Cx<R>::T *coins;
+    const typename Cx<R>::T *phases;
+    const uint8_t *broken;
+    R coin[2 * CD * CD];
+};
+
+constexpr int STEP_BLOCK = 256;
+
+template <typename R, int DIM, int KIND, bool FAST, int U>
+__global__ void __launch_bounds__(STEP_BLOCK)
+step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
+    constexpr int CD = 2 * DIM;
+    typedef typename Cx<R>::T V;
+    // block -> (walk, row m, chunk along n)
+    const long long blk = blockIdx.x;
+    const long long rowid = blk / a.chunks_per_row;
+    const int chunk = (int)(blk - rowid * a.chunks_per_row);
+    const long long w = rowid / a.box_m;
+    const long long m = a.m_lo + (rowid - w * a.box_m);
+    const long long n_base = (long long)chunk * (STEP_BLOCK * U) + threadIdx.x;
+    const long long row_off = w * a.walk_stride + m * a.pitch;
+
+    cplx<R> v[U][CD];
+    bool live[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const long long nb = n_base + (long long)u * STEP_BLOCK;
+        live[u] = nb < a.box_n;
+        if (live[u]) {
+            const long long idx = row_off + a.n_lo + nb;
+#pragma unroll
+            for (int b = 0; b < CD; ++b) v[u][b] = cx_load<R>(a.in + b * a.plane_stride + idx);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        if (!live[u]) continue;
+        const long long n = a.n_lo + n_base + (long long)u * STEP_BLOCK;
+        const long long x = m * a.en + n;
+        if constexpr (FAST) {
+            apply_coin<R, CD, KIND>(a.coin, v[u]);
+        } else {
+            if (a.coin_mode == QW_COIN_UNIFORM) {
+                apply_coin<R, CD, KIND>(a.coin, v[u]);
+            } else {
+                const long long ci = (a.coin_mode == QW_COIN_PER_WALK) ? w : (w * a.sites + x);
+                const R *Cg = reinterpret_cast<const R *>(a.coins + ci * (CD * CD));
+                R C[2 * CD * CD];
+#pragma unroll
+                for (int i = 0; i < 2 * CD * CD; ++i) C[i] = Cg[i];
+                apply_coin<R, CD, COIN_GENERAL>(C, v[u]);
+            }
+            if (a.phases) {
+                const cplx<R> ph = cx_load<R>(a.phases + w * a.sites + x);
+#pragma unroll
+                for (int c = 0; c < CD; ++c) v[u][c] = cx_mul(ph.re, ph.im, v[u][c]);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < CD; ++c) {
+            int dm, dn;
+            coin_direction<DIM>(FAST ? QW_NATURAL : a.lattice, c, dm, dn);
+            long long tm = m + dm, tn = n + dn;
+            bool stay = false;
+            if (a.boundary == QW_PERIODIC) {
+                if (DIM == 2) { if (tm < 0) tm += a.em; else if (tm >= a.em) tm -= a.em; }
+                if (tn < 0) tn += a.en; else if (tn >= a.en) tn -= a.en;
+            } else {
+                stay = (tn < 0) | (tn >= a.en);
+                if (DIM == 2) stay |= (tm < 0) | (tm >= a.em);
+            }
+            if constexpr (!FAST) {
+                if (a.broken && a.broken[(w * a.sites + x) * CD + c]) stay = true;
+            }
+            const long long dst = stay ? ((CD - 1 - c) * a.plane_stride + row_off + n)
+                                       : (c * a.plane_stride + w * a.walk_stride + tm * a.pitch + tn);
+            cx_store<R>(a.out + dst, v[u][c]);
+        }
+    }
+}
+
+// U^dagger = (I (x) C^dagger) S^dagger in gather form: the thread that owns site x reads back every
+// component from where the forward step wrote it, then applies C_x^dagger.
+template <typename R, int DIM>
+__global__ void __launch_bounds__(STEP_BLOCK)
+step_inverse_kernel(const StepArgs<R, 2 * DIM> a) {
+    constexpr int CD = 2 * DIM;
+    const long long blk = blockIdx.x;
+    const long long rowid = blk / a.chunks_per_row;
+    const int chunk = (int)(blk - rowid * a.chunks_per_row);
+    const long long w = rowid / a.em;
+    const long long m = rowid - w * a.em;
+    const long long n = (long long)chunk * STEP_BLOCK + threadIdx.x;
+    if (n >= a.en) return;
+    const long long x = m * a.en + n;
+    const long long row_off = w * a.walk_stride + m * a.pitch;
+    cplx<R> v[CD];
+#pragma unroll
+    for (int c = 0; c < CD; ++c) {
+        int dm, dn;
+        coin_direction<DIM>(a.lattice, c, dm, dn);
+        long long tm = m + dm, tn = n + dn;
+        bool stay = false;
+        if (a.boundary == QW_PERIODIC) {
+            if (DIM == 2) { if (tm < 0) tm += a.em; else if (tm >= a.em) tm -= a.em; }
+            if (tn < 0) tn += a.en; else if (tn >= a.en) tn -= a.en;
+        } else {
+            stay = (tn < 0) | (tn >= a.en);
+            if (DIM == 2) stay |= (tm < 0) | (tm >= a.em);
+        }
+        if (a.broken && a.broken[(w * a.sites + x) * CD + c]) stay = true;
+        const long long src = stay ? ((CD - 1 - c) * a.plane_stride + row_off + n)
+                                   : (c * a.plane_stride + w * a.walk_stride + tm * a.pitch + tn);
+        v[c] = cx_load<R>(a.in + src);
+    }
+    if (a.phases) {   // (ph * C)^dagger = conj(ph) * C^dagger
+        const cplx<R> ph = cx_load<R>(a.phases + w * a.sites + x);
+#pragma unroll
+        for (int c = 0; c < CD; ++c) v[c] = cx_mul(ph.re, -ph.im, v[c]);
+    }
+    R C[2 * CD * CD];
+    if (a.coin_mode == QW_COIN_UNIFORM) {
+#pragma unroll
+        for (int i = 0; i < 2 * CD * CD; ++i) C[i] = a.coin[i];
+    } else {
+        const long long ci = (a.coin_mode == QW_COIN_PER_WALK) ? w : (w * a.sites + x);
+        const R *Cg = reinterpret_cast<const R *>(a.coins + ci * (CD * CD));
+#pragma unroll
+        for (int i = 0; i < 2 * CD * CD; ++i) C[i] = Cg[i];
+    }
+    apply_coin_dagger<R, CD>(C, v);
+#pragma unroll
+    for (int b = 0; b < CD; ++b) cx_store<R>(a.out + b * a.plane_stride + row_off + n, v[b]);
+}
+
+template <typename R, int DIM>
+static void fill_args(const qw_sim *s, const void *in, void *out, const Box &box, StepArgs<R, 2 * DIM> &a) {
+    typedef typename Cx<R>::T V;
+    const Geom &g = s->g;
+    a.in = static_cast<const V *>(in);
+    a.out = static_cast<V *>(out);
+    a.em = g.em; a.en = g.en; a.pitch = g.pitch; a.walk_stride = g.walk_stride;
+    a.plane_stride = g.plane_stride; a.sites = g.sites;
+    a.m_lo = box.m_lo; a.n_lo = box.n_lo;
+    a.box_m = box.m_hi - box.m_lo + 1; a.box_n = box.n_hi - box.n_lo + 1;
+    a.boundary = g.boundary; a.lattice = g.lattice; a.coin_mode = s->coin_mode;
+    a.coins = static_cast<const V *>(s->d_coin);
+    a.phases = static_cast<const V *>(s->d_phases);
+    a.broken = s->d_broken;
+    for (int i = 0; i < 2 * g.cdim * g.cdim; ++i) a.coin[i] = (R)s->h_coin[i];
+}
+
+template <typename R, int DIM, int KIND, bool FAST, int U>
+static int launch_scatter(qw_sim *s, StepArgs<R, 2 * DIM> &a) {
+    const long long per_block = (long long)STEP_BLOCK * U;
+    a.chunks_per_row = (int)((a.box_n + per_block - 1) / per_block);
+    const long long blocks = s->g.batch * a.box_m * a.chunks_per_row;
+    if (blocks <= 0) return QW_OK;
+    if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
+    step_scatter_kernel<R, DIM, KIND, FAST, U><<<(unsigned)blocks, STEP_BLOCK, 0, s->stream>>>(a);
+    QW_LAUNCH_CHECK(s, "step_scatter_kernel");
+    return QW_OK;
+}
+
+template <typename R, int DIM>
+static int launch_step_t(qw_sim *s, const void *in, void *out, const Box &box, bool allow_fast) {
+    StepArgs<R, 2 * DIM> a;
+    fill_args<R, DIM>(s, in, out, box, a);
+    const bool fast = allow_fast && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
+                      s->g.lattice == QW_NATURAL;
+    // U sites per thread: 128 B of loads in flight per thread
+    constexpr int UF = (DIM == 1) ? (sizeof(R) == 8 ? 4 : 8) : (sizeof(R) == 8 ? 2 : 4);
+    if (fast) {
+        switch (s->coin_kind) {
+            case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, true, UF>(s, a); break;
+            case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, true, UF>(s, a); break;
+            case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, true, UF>(s, a); break;
+            case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, true, UF>(s, a); break;
+            default: break;
+        }
+        return launch_scatter<R, DIM, COIN_GENERAL, true, UF>(s, a);
+    }
+    // the general kernel keeps the coin kind of the uniform matrix so that schedules agree bit for bit
+    if (s->coin_mode == QW_COIN_UNIFORM) {
+        switch (s->coin_kind) {
+            case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, false, 1>(s, a); break;
+            case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, false, 1>(s, a); break;
+            case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, false, 1>(s, a); break;
+            case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, false, 1>(s, a); break;
+            default: break;
+        }
+    }
+    return launch_scatter<R, DIM, COIN_GENERAL, false, 1>(s, a);
+}
+
+int launch_step(qw_sim *s, const void *in, void *out, const Box &box, bool allow_fast) {
+    if (s->dtype == QW_C128)
+        return s->g.dim == 1 ? launch_step_t<double, 1>(s, in, out, box, allow_fast)
+                             : launch_step_t<double, 2>(s, in, out, box, allow_fast);
+    return s->g.dim == 1 ? launch_step_t<float, 1>(s, in, out, box, allow_fast)
+                         : launch_step_t<float, 2>(s, in, out, box, allow_fast);
+}
+
+template <typename R, int DIM>
+static int launch_inverse_t(qw_sim *s, const void *in, void *out) {
+    StepArgs<R, 2 * DIM> a;
+    Box full{0, s->g.em - 1, 0, s->g.en - 1};
+    fill_args<R, DIM>(s, in, out, full, a);
+    a.chunks_per_row = (int)((s->g.en + STEP_BLOCK - 1) / STEP_BLOCK);
+    const long long blocks = s->g.batch * s->g.em * a.chunks_per_row;
+    if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
+    step_inverse_kernel<R, DIM><<<(unsigned)blocks, STEP_BLOCK, 0, s->stream>>>(a);
+    QW_LAUNCH_CHECK(s, "step_inverse_kernel");
+    return QW_OK;
+}
+
+int launch_step_inverse(qw_sim *s, const void *in, void *out) {
+    if (s->dtype == QW_C128)
+        return s->g.dim == 1 ? launch_inverse_t<double, 1>(s, in, out) : launch_inverse_t<double, 2>(s, in, out);
+    return s->g.dim == 1 ? launch_inverse_t<float, 1>(s, in, out) : launch_inverse_t<float, 2>(s, in, out);
+}
+
+}  // namespace qw

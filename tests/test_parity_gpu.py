@@ -1,0 +1,316 @@
+"""GPU parity: libqw (through the C ABI, via the ctypes binding) against the CPU oracle, element by
+element on the same seeded inputs.  Gates (BASELINE.json:north_star):
+    complex128   max |d amplitude| <= 1e-12, |d probability| <= 1e-12 per site
+    complex64    max |d amplitude| <= 2e-5, |1 - norm| <= 1e-4 after the full step count
+    moments      complex128 relative 1e-10; complex64 relative 1e-4          (R24)
+The oracle always runs in double on exactly the bytes the library received (for complex64: the
+float-rounded state and coin promoted to double, R21).
+"""
+import numpy as np
+import pytest
+
+from paper_1003_3779_b200 import inputs as qi
+
+pytestmark = pytest.mark.gpu
+
+AMP_TOL = {np.dtype(np.complex128): 1e-12, np.dtype(np.complex64): 2e-5}
+MOM_RTOL = {np.dtype(np.complex128): 1e-10, np.dtype(np.complex64): 1e-4}
+
+
+@pytest.fixture(scope="module")
+def dev(qw):
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    torch.cuda.init()
+    return torch.device("cuda:0")
+
+
+def real_dtype(w):
+    return np.float64 if w.dtype == np.complex128 else np.float32
+
+
+def gpu_run(qw, w, steps=None, schedule=None, k=0, window=True, inverse=0, broken=None, get_state=True):
+    """Run workload w on the GPU; returns (amps AoS in w.dtype, P, moments, info)."""
+    steps = w.steps if steps is None else steps
+    h = qw.create_for(w)
+    try:
+        if broken is not None:
+            qw.qw_set_broken_links(h, broken)
+        if schedule is not None:
+            qw.qw_set_schedule(h, schedule, k)
+        qw.qw_set_window(h, window)
+        qw.load_state(h, w)
+        qw.qw_step(h, steps)
+        if inverse:
+            qw.qw_step_inverse(h, inverse)
+        amps = None
+        if get_state:
+            amps = np.empty((w.batch, w.sites, w.coin_dim), dtype=w.dtype)
+            qw.qw_get_state(h, amps)
+        P = np.empty((w.batch, w.sites), dtype=real_dtype(w))
+        qw.qw_probabilities(h, P)
+        mom = np.empty((w.batch, 3 if w.dim == 1 else 6), dtype=np.float64)
+        qw.qw_moments(h, mom)
+        info = {"launches": qw.qw_get_info(h, qw.QW_INFO_LAUNCHES), "sched": qw.qw_get_info(h, qw.QW_INFO_LAST_SCHEDULE),
+                "k": qw.qw_get_info(h, qw.QW_INFO_LAST_K), "t": qw.qw_get_info(h, qw.QW_INFO_TIME)}
+        return amps, P, mom, info
+    finally:
+        qw.qw_destroy(h)
+
+
+def oracle_run(oracle, w, steps=None, inverse=0, broken=None):
+    steps = w.steps if steps is None else steps
+    mode, coin = w.general_coin_f64()
+    psi = np.ascontiguousarray(w.initial_state().astype(np.complex128))
+    kw = dict(boundary=w.boundary, coin_mode=mode, batch=w.batch, lattice=w.lattice, broken=broken)
+    oracle.step(w.extents, coin, psi, steps, **kw)
+    if inverse:
+        oracle.step_inverse(w.extents, coin, psi, inverse, **kw)
+    return psi, oracle.probabilities(w.extents, psi, batch=w.batch), oracle.moments(w.extents, psi, batch=w.batch)
+
+
+def check_parity(w, gpu, ora, mom_abs_mean=None):
+    amps, P, mom, _ = gpu
+    psi, Po, momo = ora
+    tol = AMP_TOL[np.dtype(w.dtype)]
+    if amps is not None:
+        d = np.max(np.abs(amps.astype(np.complex128) - psi)) if psi.size else 0.0
+        assert d <= tol, "max |d amplitude| = %.3e > %.1e" % (d, tol)
+    ptol = 1e-12 if w.dtype == np.complex128 else 4 * w.coin_dim * tol
+    dP = np.max(np.abs(P.astype(np.float64) - Po)) if Po.size else 0.0
+    assert dP <= ptol, "max |d probability| = %.3e" % dP
+    rt = MOM_RTOL[np.dtype(w.dtype)]
+    ext = max(w.extents)
+    nm = 1 if w.dim == 1 else 2
+    for b in range(w.batch):
+        assert abs(mom[b, 0] - momo[b, 0]) <= rt * abs(momo[b, 0]), ("norm", mom[b, 0], momo[b, 0])
+        for j in range(1, 1 + nm):                                   # means: absolute rt*extent where mean ~ 0
+            assert abs(mom[b, j] - momo[b, j]) <= rt * (abs(momo[b, j]) + ext), ("mean", mom[b], momo[b])
+        second = 1.0 + max(abs(momo[b, j]) for j in range(1 + nm, mom.shape[1])) + max(momo[b, j] ** 2 for j in range(1, 1 + nm))
+        for j in range(1 + nm, mom.shape[1]):                        # variances / covariance: relative to E[x^2]
+            assert abs(mom[b, j] - momo[b, j]) <= rt * second, ("second moment", j, mom[b], momo[b])
+    if w.dtype == np.complex64:
+        assert np.max(np.abs(1 - mom[:, 0])) <= 1e-4
+
+
+# ------------------------------------------------------------------ the five configs, scaled twins
+def test_k0_exact_config(qw, oracle, dev):
+    w = qi.k0()
+    gpu = gpu_run(qw, w)
+    check_parity(w, gpu, oracle_run(oracle, w))
+    P = gpu[1][0]
+    assert np.max(np.abs(P - P[::-1])) <= 1e-15                      # P5 symmetry on the GPU too
+    assert np.all(P[(np.arange(-100, 101) + 100) % 2 == 1] == 0.0)   # P4 exact zeros
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("sites,steps", [(1 << 16, 200), (100003, 64), (1024 * 4 * 3 + 1, 33)])
+def test_k1_ring_twins(qw, oracle, dev, dtype, sites, steps):
+    w = qi.k1(sites=sites, steps=steps, dtype=dtype)
+    check_parity(w, gpu_run(qw, w), oracle_run(oracle, w))
+
+
+@pytest.mark.parametrize("half,steps", [(64, 64), (40, 100)])
+def test_k2_grover_twins(qw, oracle, dev, half, steps):
+    w = qi.k2(half=half, steps=steps)                                # steps > half: the wall reflects
+    gpu = gpu_run(qw, w)
+    check_parity(w, gpu, oracle_run(oracle, w))
+    if steps <= half:
+        P = gpu[1][0].reshape(w.extents)
+        assert np.array_equal(P, P[::-1, :]) and np.array_equal(P, P.T)
+
+
+@pytest.mark.parametrize("coin", ["hxh", "dft", "grover"])
+@pytest.mark.parametrize("extents,steps", [((256, 256), 50), ((61, 35), 40), ((8, 1030), 25)])
+def test_k3_torus_twins(qw, oracle, dev, coin, extents, steps):
+    w = qi.k3(extents=extents, steps=steps, coin=coin)
+    check_parity(w, gpu_run(qw, w), oracle_run(oracle, w))
+
+
+@pytest.mark.parametrize("batch,half,steps", [(16, 64, 64), (5, 21, 100), (3, 1024, 40)])
+def test_k4_batch_twins(qw, oracle, dev, batch, half, steps):
+    w = qi.k4(batch=batch, half=half, steps=steps)
+    check_parity(w, gpu_run(qw, w), oracle_run(oracle, w))
+
+
+# ------------------------------------------------------------------ feature matrix on small lattices
+def small_workload(dim, boundary, dtype, coin_mode, rng, lattice=qi.NATURAL, phases=False, batch=2, extents=None):
+    ext = extents if extents is not None else ((37,) if dim == 1 else (11, 14))
+    sites = int(np.prod(ext))
+    cd = 2 * dim
+    if coin_mode == qi.COIN_UNIFORM:
+        coin = qi.random_unitary(rng, cd)
+    elif coin_mode == qi.COIN_PER_WALK:
+        coin = np.stack([qi.random_unitary(rng, cd) for _ in range(batch)])
+    else:
+        coin = np.stack([qi.random_unitary(rng, cd) for _ in range(batch * sites)]).reshape(batch, sites, cd, cd)
+    ph = np.exp(1j * rng.uniform(0, 2 * np.pi, (batch, sites))).astype(dtype) if phases else None
+    return qi.Workload("small", dim, tuple(ext), batch, boundary, np.dtype(dtype), 30, coin_mode,
+                       coin.astype(dtype), phases=ph,
+                       state=qi.random_state(77, batch, sites, cd, dtype, normalise_per_walk=True), lattice=lattice)
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+@pytest.mark.parametrize("dim", [1, 2])
+@pytest.mark.parametrize("coin_mode,phases", [(qi.COIN_UNIFORM, False), (qi.COIN_UNIFORM, True),
+                                              (qi.COIN_PER_WALK, True), (qi.COIN_PER_SITE, False)])
+def test_feature_matrix(qw, oracle, dev, dtype, boundary, dim, coin_mode, phases):
+    rng = np.random.default_rng(100 + 10 * dim + boundary)
+    w = small_workload(dim, boundary, dtype, coin_mode, rng, phases=phases)
+    check_parity(w, gpu_run(qw, w), oracle_run(oracle, w))
+
+
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+def test_diagonal_lattice(qw, oracle, dev, boundary, dtype):
+    rng = np.random.default_rng(5)
+    w = small_workload(2, boundary, dtype, qi.COIN_UNIFORM, rng, lattice=qi.DIAGONAL)
+    check_parity(w, gpu_run(qw, w), oracle_run(oracle, w))
+
+
+@pytest.mark.parametrize("dim,lattice", [(1, qi.NATURAL), (2, qi.NATURAL), (2, qi.DIAGONAL)])
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+def test_static_broken_links(qw, oracle, dev, dim, lattice, boundary):
+    rng = np.random.default_rng(6)
+    w = small_workload(dim, boundary, np.complex128, qi.COIN_UNIFORM, rng, lattice=lattice)
+    mask = qi.symmetric_broken_links(qi.SEED_RBL, dim, w.extents, w.batch, 0.25, boundary, lattice)
+    gpu = gpu_run(qw, w, broken=mask)
+    check_parity(w, gpu, oracle_run(oracle, w, broken=mask))
+    assert np.max(np.abs(gpu[2][:, 0] - 1)) < 1e-13                  # still unitary
+
+
+@pytest.mark.parametrize("extents", [(1,), (2,), (3,), (1, 1), (1, 5), (5, 1), (2, 2), (2, 3)])
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+def test_degenerate_extents(qw, oracle, dev, extents, boundary):
+    rng = np.random.default_rng(8)
+    for dtype in (np.complex128, np.complex64):
+        w = small_workload(len(extents), boundary, dtype, qi.COIN_UNIFORM, rng, batch=3, extents=extents)
+        check_parity(w, gpu_run(qw, w), oracle_run(oracle, w))
+
+
+# ------------------------------------------------------------------ inverse step / reversibility (P6)
+@pytest.mark.parametrize("dim", [1, 2])
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+def test_inverse_step(qw, oracle, dev, dim, boundary):
+    rng = np.random.default_rng(9)
+    w = small_workload(dim, boundary, np.complex128, qi.COIN_PER_WALK, rng, phases=True)
+    check_parity(w, gpu_run(qw, w, steps=7, inverse=3), oracle_run(oracle, w, steps=7, inverse=3))
+    amps, _, _, info = gpu_run(qw, w, steps=100, inverse=100)
+    assert info["t"] == 0
+    assert np.max(np.abs(amps - w.initial_state())) <= 1e-13
+
+
+# ------------------------------------------------------------------ schedule / window invariance (P13), P12
+def test_generic_and_fused_schedules_agree_bit_for_bit(qw, dev):
+    for w in (qi.k1(sites=50021, steps=40), qi.k1(sites=50021, steps=40, dtype=np.complex64),
+              qi.k3(extents=(97, 130), steps=20, coin="dft"), qi.k3(extents=(97, 130), steps=20, coin="hxh"),
+              qi.k2(half=33, steps=50)):
+        a = gpu_run(qw, w, schedule=qw.QW_SCHED_GENERIC)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        assert a[3]["sched"] == qw.QW_SCHED_GENERIC and b[3]["sched"] == qw.QW_SCHED_FUSED
+        assert np.array_equal(a[0], b[0]), w.name
+
+
+@pytest.mark.parametrize("wl", ["k0", "k2", "k4", "k2-periodic-corner"])
+def test_light_cone_window_is_exact(qw, dev, wl):
+    """the 'line' variant updates only the sites the walker can have reached."""
+    if wl == "k0":
+        w = qi.k0(steps=130, half_width=100)          # front reaches the wall at step 100, then reflects
+    elif wl == "k2":
+        w = qi.k2(half=30, steps=45)
+    elif wl == "k4":
+        w = qi.k4(batch=4, half=40, steps=60)
+    else:
+        w = qi.k2(half=20, steps=30)
+        w.boundary = qi.PERIODIC
+        w.delta_site = (1, 39)                        # window wraps at once in both directions
+    on = gpu_run(qw, w, window=True)
+    off = gpu_run(qw, w, window=False)
+    assert np.array_equal(on[0], off[0])
+    assert np.array_equal(on[1], off[1])
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+def test_translation_covariance_bit_exact(qw, dev, dtype):
+    """P12: on a periodic lattice with a uniform coin, shifting psi0 by s sites shifts psi(t) by s."""
+    w = qi.k1(sites=40000, steps=50, dtype=dtype)
+    a = gpu_run(qw, w)[0]
+    w2 = qi.k1(sites=40000, steps=50, dtype=dtype)
+    w2.state = np.ascontiguousarray(np.roll(w.state, 12345, axis=1))
+    b = gpu_run(qw, w2)[0]
+    assert np.array_equal(np.roll(a, 12345, axis=1), b)
+    w = qi.k3(extents=(96, 200), steps=30, coin="dft", dtype=dtype)
+    a = gpu_run(qw, w)[0].reshape(96, 200, 4)
+    w2 = qi.k3(extents=(96, 200), steps=30, coin="dft", dtype=dtype)
+    w2.state = np.ascontiguousarray(np.roll(w.state.reshape(96, 200, 4), (37, 101), axis=(0, 1)).reshape(1, -1, 4))
+    b = gpu_run(qw, w2)[0].reshape(96, 200, 4)
+    assert np.array_equal(np.roll(a, (37, 101), axis=(0, 1)), b)
+
+
+# ------------------------------------------------------------------ boundary behaviour: pointers, streams, errors
+def test_device_pointers_and_user_stream(qw, oracle, dev):
+    import torch
+    w = qi.k3(extents=(64, 96), steps=12, coin="dft")
+    stream = torch.cuda.Stream()
+    h = qw.create_for(w)
+    try:
+        qw.qw_set_stream(h, stream.cuda_stream)
+        with torch.cuda.stream(stream):
+            st = torch.from_numpy(w.state).to(dev, non_blocking=False)
+            qw.qw_set_state(h, st)
+            qw.qw_step(h, w.steps)
+            out = torch.empty((w.batch, w.sites, 4), dtype=torch.complex64, device=dev)
+            P = torch.empty((w.batch, w.sites), dtype=torch.float32, device=dev)
+            mom = torch.empty((w.batch, 6), dtype=torch.float64, device=dev)
+            qw.qw_get_state(h, out); qw.qw_probabilities(h, P); qw.qw_moments(h, mom)
+        qw.qw_synchronize(h)
+        stream.synchronize()
+        gpu = (out.cpu().numpy(), P.cpu().numpy(), mom.cpu().numpy(), None)
+    finally:
+        qw.qw_destroy(h)
+    check_parity(w, gpu, oracle_run(oracle, w))
+
+
+def test_error_codes_on_device(qw, dev):
+    h = qw.qw_create(1, [64], 2, qw.QW_C128, qw.QW_OPEN)
+    try:
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_step(h, 1)
+        assert ei.value.code == qw.QW_ESTATE                        # no coin yet
+        qw.qw_set_coin(h, qw.QW_COIN_UNIFORM, qi.hadamard())
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_step(h, 1)
+        assert ei.value.code == qw.QW_ESTATE                        # no state yet
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_set_state_delta(h, [64], np.array([1, 0], dtype=np.complex128))
+        assert ei.value.code == qw.QW_EINVAL
+        qw.qw_set_state_delta(h, [32], np.array([1, 0], dtype=np.complex128))
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_step(h, -1)
+        assert ei.value.code == qw.QW_EINVAL
+        qw.qw_step(h, 0)
+        assert qw.qw_get_info(h, qw.QW_INFO_TIME) == 0
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_set_lattice(h, qw.QW_DIAGONAL)
+        assert ei.value.code == qw.QW_EINVAL
+        with pytest.raises(qw.QwError):
+            qw.qw_set_coin(h, 9, qi.hadamard())
+    finally:
+        qw.qw_destroy(h)
+
+
+def test_set_state_round_trip_is_exact(qw, dev):
+    for dtype in (np.complex128, np.complex64):
+        for ext, batch in (((1001,), 3), ((33, 47), 2)):
+            sites = int(np.prod(ext))
+            st = qi.random_state(5, batch, sites, 2 * len(ext), dtype)
+            h = qw.qw_create_batch(batch, len(ext), ext, 2 * len(ext), qw.dtype_code(dtype), qw.QW_PERIODIC)
+            try:
+                qw.qw_set_state(h, st)
+                back = np.empty_like(st)
+                qw.qw_get_state(h, back)
+                assert np.array_equal(back, st)
+            finally:
+                qw.qw_destroy(h)
