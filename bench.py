@@ -1,0 +1,474 @@
+#!/usr/bin/env python
+"""bench.py — site-updates/s of the quantum-walk hot path on B200 (BASELINE.json:metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload k1|k1c64|k2|k3hxh|k3dft|k4]
+    python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N ...
+    python bench.py --impl reference ...          # the CPU oracle, as it stands, on the host cores
+
+One bench "step" is one pass of the whole hot path over the resident workload: qw_step(walk_steps)
+(coin + conditional shift, eq. 2) followed by the workload's outputs (qw_moments and/or
+qw_probabilities).  The default workload is BASELINE.json:configs[1] (K1: 1D Hadamard
+ring of 2^26 sites, complex128, 1000 walk steps, norm/mean/variance) — the configuration the
+metric is quoted on; the other configs are reachable with --workload (parity-tested in tests/).
+The state (2 x 2 GiB ping-pong) is far larger than the 126 MB L2, so no explicit L2 flush is needed.
+
+Multi-GPU: the north_star forbids sharding ("no sharding across GPUs, no collectives"), so
+--gpus N runs N independent replicas; value is the
+aggregate over replicas and the time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1003_3779_b200 import inputs as qi  # noqa: E402
+
+METRIC = "site-updates/s"
+FALLBACK_HBM_GBS = 6650.0    # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+# ----------------------------------------------------------------------------------------------
+def make_workload(name: str, walk_steps=None):
+    if name == "k1":
+        return qi.k1(steps=walk_steps or 1000)
+    if name == "k1c64":
+        return qi.k1(steps=walk_steps or 1000, dtype=np.complex64)
+    if name == "k2":
+        return qi.k2(steps=walk_steps)
+    if name == "k3hxh":
+        return qi.k3(steps=walk_steps or 500, coin="hxh")
+    if name == "k3dft":
+        return qi.k3(steps=walk_steps or 500, coin="dft")
+    if name == "k4":
+        return qi.k4(steps=walk_steps)
+    if name == "k0":
+        return qi.k0(steps=walk_steps or 100)
+    raise SystemExit("unknown workload %r" % name)
+
+
+def workload_config(name, w, extra=None):
+    cfg = {
+        "workload": "%s: %dD %s lattice %s, batch %d, %s, coin %s, %d walk steps per bench step, outputs %s"
+                    % (w.name, w.dim, "periodic" if w.boundary == qi.PERIODIC else "open",
+                       "x".join(str(e) for e in w.extents), w.batch, np.dtype(w.dtype).name,
+                       {0: "uniform", 1: "per-walk", 2: "per-site"}[w.coin_mode] + ("+site-phases" if w.phases is not None else ""),
+                       w.steps, "+".join(w.outputs)),
+        "baseline_config": {"k0": 0, "k1": 1, "k1c64": 1, "k2": 2, "k3hxh": 3, "k3dft": 3, "k4": 4}[name],
+        "sites": w.sites, "batch": w.batch, "walk_steps": w.steps,
+        "l2": "working set (2 ping-pong state buffers) exceeds the 126 MB L2; no flush needed"
+              if 2 * w.sites * w.batch * w.coin_dim * np.dtype(w.dtype).itemsize > 2 * 126e6 else
+              "state fits in L2/SM: resident workload, HBM is touched only at the ends",
+        "parallelism": "replicas",
+    }
+    if extra:
+        cfg.update(extra)
+    return cfg
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def stored_traffic(name):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(name)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------------------------
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def init_dist(backend: str):
+    """Initialise torch.distributed from the torchrun environment (127.0.0.1 rendezvous)."""
+    import torch.distributed as dist
+    rank, world, _ = dist_env()
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, world
+
+
+def barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def max_over_ranks(value: float, world: int, device=None) -> float:
+    """MAX of a per-rank scalar (device time in ms): the job is as slow as its slowest replica."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(value: float, world: int, device=None) -> float:
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def aggregate_rate(units_per_rank: float, ms_per_rank: float, world: int, device=None):
+    """Whole-job rate: units all ranks processed / max-over-ranks time."""
+    ms = max_over_ranks(ms_per_rank, world, device)
+    units = sum_over_ranks(units_per_rank, world, device)
+    return units / (ms * 1e-3), ms
+
+
+# ----------------------------------------------------------------------------------------------
+def oracle_sample(name: str, w, seconds_target: float = 12.0):
+    """Time the CPU oracle, as it stands, on a bounded sample of workload `name` (1 thread)."""
+    import oracle
+    oracle.build()
+    if name in ("k1", "k1c64"):
+        sw = qi.k1(log2_sites=22, steps=8, dtype=w.dtype)
+        desc = "same ring workload cut to 2^22 sites x %d walk steps"
+    elif name == "k2":
+        sw = qi.k2(half=512, steps=4)
+        desc = "same open Grover lattice cut to 1025^2 sites x %d walk steps"
+    elif name in ("k3hxh", "k3dft"):
+        sw = qi.k3(extent=1024, steps=4, coin=name[2:])
+        desc = "same torus workload cut to 1024^2 sites x %d walk steps"
+    elif name == "k4":
+        sw = qi.k4(batch=64, half=1024, steps=32)
+        desc = "64 of the 4096 walks x %d walk steps"
+    else:
+        sw = qi.k0()
+        desc = "the whole config (%d walk steps)"
+    mode, coin = sw.general_coin_f64()
+    psi = np.ascontiguousarray(sw.initial_state().astype(np.complex128))
+    kw = dict(boundary=sw.boundary, coin_mode=mode, batch=sw.batch)
+    # calibrate: one short call, then scale the step count to ~seconds_target
+    t0 = time.perf_counter(); oracle.step(sw.extents, coin, psi, 1, **kw); t1 = time.perf_counter() - t0
+    steps = int(max(1, min(4096, seconds_target / max(t1, 1e-6))))
+    t0 = time.perf_counter(); oracle.step(sw.extents, coin, psi, steps, **kw); dt = time.perf_counter() - t0
+    if "probabilities" in sw.outputs:
+        oracle.probabilities(sw.extents, psi, batch=sw.batch)
+    if "moments" in sw.outputs:
+        oracle.moments(sw.extents, psi, batch=sw.batch)
+    rate = sw.sites * sw.batch * steps / dt
+    return {"value": rate, "unit": METRIC, "cores": 1, "kind": "oracle",
+            "sample": (desc % steps) + ", single thread, g++ -O2 (oracle/qw_oracle.cpp)",
+            "seconds": dt, "host_cores_available": os.cpu_count()}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/config keys (rank 0 only)."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    w_desc = make_workload(args.workload, args.walk_steps) if args.workload in ("k0",) else None
+    # describe the workload without materialising the 2 GiB state
+    names = {"k1": ("K1", 1, (1 << 26,), 1, np.complex128, 1000), "k1c64": ("K1", 1, (1 << 26,), 1, np.complex64, 1000)}
+    import oracle
+    oracle.build()
+    if args.workload in ("k1", "k1c64"):
+        dtype = np.complex128 if args.workload == "k1" else np.complex64
+        sw = qi.k1(log2_sites=22, steps=4, dtype=dtype)
+        sample = "ring cut to 2^22 sites, 4 walk steps per bench step (oracle: double precision, 1 thread)"
+        full_sites, full_batch, full_steps = 1 << 26, 1, args.walk_steps or 1000
+        wl_name = "K1"
+    else:
+        sw = {"k2": lambda: qi.k2(half=512, steps=2), "k3hxh": lambda: qi.k3(extent=1024, steps=2, coin="hxh"),
+              "k3dft": lambda: qi.k3(extent=1024, steps=2, coin="dft"), "k4": lambda: qi.k4(batch=64, steps=16),
+              "k0": lambda: qi.k0()}[args.workload]()
+        sample = "%s cut to %d sites x batch %d, %d walk steps per bench step" % (sw.name, sw.sites, sw.batch, sw.steps)
+        full_sites, full_batch, full_steps = sw.sites, sw.batch, sw.steps
+        wl_name = sw.name
+    mode, coin = sw.general_coin_f64()
+    psi = np.ascontiguousarray(sw.initial_state().astype(np.complex128))
+    kw = dict(boundary=sw.boundary, coin_mode=mode, batch=sw.batch)
+
+    def one():
+        oracle.step(sw.extents, coin, psi, sw.steps, **kw)
+        if "moments" in sw.outputs:
+            oracle.moments(sw.extents, psi, batch=sw.batch)
+        if "probabilities" in sw.outputs:
+            oracle.probabilities(sw.extents, psi, batch=sw.batch)
+
+    for _ in range(args.warmup):
+        one()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        one()
+    dt = time.perf_counter() - t0
+    rate = sw.sites * sw.batch * sw.steps * args.steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": METRIC, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s (BASELINE.json configs[%d]); reference arm = CPU oracle on a bounded sample: %s"
+                               % (wl_name, {"k0": 0, "k1": 1, "k1c64": 1, "k2": 2, "k3hxh": 3, "k3dft": 3, "k4": 4}[args.workload], sample),
+                   "sites": full_sites, "batch": full_batch, "walk_steps": full_steps, "parallelism": "replicas"},
+        "cpu_baseline": {"value": rate, "unit": METRIC, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------
+def run_gpu(args):
+    import torch
+    from paper_1003_3779_b200 import binding as qw
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libqw has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    init_dist("nccl")
+    qw.load()
+
+    w = make_workload(args.workload, args.walk_steps)
+    real = np.float64 if w.dtype == np.complex128 else np.float32
+    ebytes = np.dtype(w.dtype).itemsize
+    site_updates_per_step = float(w.sites) * w.batch * w.steps
+    alg_bytes_per_site = 2 * w.coin_dim * ebytes          # read + write every amplitude once
+
+    h = qw.create_for(w)
+    if args.schedule is not None:
+        qw.qw_set_schedule(h, {"auto": 0, "generic": 1, "fused": 2, "blocked": 3, "resident": 4}[args.schedule], args.k)
+    if args.no_window:
+        qw.qw_set_window(h, 0)
+    stream = torch.cuda.current_stream()
+    qw.qw_set_stream(h, stream.cuda_stream)
+
+    # outputs on the device; host-pinned copies for the end-to-end leg
+    mom_d = torch.empty((w.batch, 3 if w.dim == 1 else 6), dtype=torch.float64, device=dev)
+    P_d = torch.empty((w.batch, w.sites), dtype=torch.float64 if real == np.float64 else torch.float32, device=dev) \
+        if "probabilities" in w.outputs else None
+
+    def outputs_device():
+        if "moments" in w.outputs:
+            qw.qw_moments(h, mom_d)
+        if P_d is not None:
+            qw.qw_probabilities(h, P_d)
+
+    # ---- device-resident leg ------------------------------------------------------------------
+    # Random-state workloads (K1, K3) keep evolving the resident state; delta-start workloads (K0, K2,
+    # K4) restart from the delta every bench step (a device-side memset + one tiny kernel) so that
+    # every bench step IS the config: the walker starts at the centre and never reaches the boundary.
+    delta = w.state is None
+    delta_coin = np.ascontiguousarray(w.delta_coin, dtype=w.dtype) if delta else None
+
+    def hot_path():
+        if delta:
+            qw.qw_set_state_delta(h, w.delta_site, delta_coin)
+        qw.qw_step(h, w.steps)
+
+    qw.load_state(h, w)
+    for _ in range(max(args.warmup, 3)):
+        hot_path()
+        outputs_device()
+    torch.cuda.synchronize()
+    barrier(world)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    l0 = qw.qw_get_info(h, qw.QW_INFO_LAUNCHES)
+    torch.cuda.synchronize()
+    for i in range(args.steps):
+        ev[i][0].record(stream)
+        hot_path()
+        ev[i][1].record(stream)
+        outputs_device()
+        ev[i][2].record(stream)
+    torch.cuda.synchronize()
+    barrier(world)
+    clocks = sampler.stop() if rank == 0 else None
+    launches = qw.qw_get_info(h, qw.QW_INFO_LAUNCHES) - l0
+    total_ms = ev[0][0].elapsed_time(ev[-1][2])
+    step_ms = sum(e[0].elapsed_time(e[1]) for e in ev)
+    out_ms = sum(e[1].elapsed_time(e[2]) for e in ev)
+    sched = qw.qw_get_info(h, qw.QW_INFO_LAST_SCHEDULE)
+    kdepth = qw.qw_get_info(h, qw.QW_INFO_LAST_K)
+    windowed = qw.qw_get_info(h, qw.QW_INFO_WINDOW)
+    value, ms = aggregate_rate(site_updates_per_step * args.steps, total_ms, world, dev)
+    qw.qw_moments(h, mom_d)
+    mom_host = mom_d.cpu().numpy()
+
+    # ---- end-to-end leg: host buffers, H2D + D2H inside the timed region -----------------------
+    e2e = None
+    if not args.no_e2e:
+        init = w.initial_state()
+        st_pin = torch.from_numpy(init).pin_memory()
+        mom_pin = torch.empty((w.batch, mom_d.shape[1]), dtype=torch.float64).pin_memory()
+        P_pin = torch.empty((w.batch, w.sites), dtype=P_d.dtype).pin_memory() if P_d is not None else None
+        h2d = st_pin.numel() * st_pin.element_size()
+        d2h = (mom_pin.numel() * 8 if "moments" in w.outputs else 0) + (P_pin.numel() * P_pin.element_size() if P_pin is not None else 0)
+
+        def e2e_step():
+            qw.qw_set_state(h, st_pin)                    # H2D copy + layout kernel (general state: no window)
+            qw.qw_step(h, w.steps)
+            if "moments" in w.outputs:
+                qw.qw_moments(h, mom_pin)                 # D2H, synchronises
+            if P_pin is not None:
+                qw.qw_probabilities(h, P_pin)
+
+        e2e_step()
+        torch.cuda.synchronize(); barrier(world)
+        n_e2e = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n_e2e):
+            e2e_step()
+        b.record(stream)
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        e2e_ms = max(a.elapsed_time(b), wall_ms)          # host-synchronous pieces count too
+        barrier(world)
+        e_val, e_ms = aggregate_rate(site_updates_per_step * n_e2e, e2e_ms, world, dev)
+        e2e = {"value": e_val, "unit": METRIC, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": e_ms / n_e2e, "steps": n_e2e, "api": "qw_set_state(host) + qw_step + qw_moments/qw_probabilities(host)"}
+    qw.qw_destroy(h)
+
+    if rank != 0:
+        return 0
+    peak, peak_src = measured_peak()
+    n_step_launches = w.steps * args.steps if kdepth <= 1 else None
+    kernel_ms = step_ms / args.steps            # device time of qw_step(walk_steps), gaps included
+    eff_gbs = site_updates_per_step * alg_bytes_per_site / (kernel_ms * 1e-3) / 1e9
+    sched_name = {0: "auto", 1: "generic", 2: "fused", 3: "blocked", 4: "resident"}.get(sched, str(sched))
+    roofline = {
+        "bound": "hbm" if sched in (1, 2) else "alu",
+        "kernel": {1: "step_scatter_kernel (generic)", 2: "step_scatter_kernel (fused coin+shift)",
+                   3: "step_blocked_kernel", 4: "step_resident_kernel"}.get(sched, "?"),
+        "achieved": eff_gbs, "peak": peak, "unit": "GB/s", "frac": eff_gbs / peak,
+        "peak_source": "of " + peak_src,
+        "frac_of_nominal_8000": eff_gbs / 8000.0,
+        "algorithmic_bytes_per_site_step": alg_bytes_per_site,
+        "avg_launch_ms": (step_ms / (w.steps * args.steps)) if kdepth <= 1 else None,
+        "traffic": stored_traffic(args.workload),
+        "note": "achieved = 2*coin_dim*sizeof(complex) bytes x site-updates / CUDA-event time of qw_step; "
+                "for blocked/resident schedules this is the EFFECTIVE bandwidth (may exceed the HBM peak)",
+    }
+    line = {
+        "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if w.dtype == np.complex128 else "f32",
+        "data": "synthetic",
+        "config": workload_config(args.workload, w, {"schedule": sched_name, "k": kdepth, "window": bool(windowed),
+                                                     "step_ms": step_ms / args.steps, "outputs_ms": out_ms / args.steps}),
+        "effective_hbm_gbs": eff_gbs,
+        "roofline": roofline,
+        "clocks": clocks,
+        "gpu_launches": int(launches),
+        "e2e": e2e,
+        "result": {"norm": float(mom_host[0, 0]), "mean": float(mom_host[0, 1]), "var": float(mom_host[0, -1] if w.dim == 1 else mom_host[0, 3])},
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = oracle_sample(args.workload, w)
+    elif world > 1:
+        line["cpu_baseline"] = None
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="k1", choices=["k0", "k1", "k1c64", "k2", "k3hxh", "k3dft", "k4"])
+    ap.add_argument("--walk-steps", type=int, default=None, help="walk steps per bench step (default: the config's)")
+    ap.add_argument("--schedule", default=None, choices=["auto", "generic", "fused", "blocked", "resident"])
+    ap.add_argument("--k", type=int, default=0)
+    ap.add_argument("--no-window", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
