@@ -350,10 +350,41 @@ int qw_step(qw_sim *s, int64_t n) {
     if (!s->has_coin) return fail(QW_ESTATE, "qw_step before qw_set_coin");
     if (!s->has_state) return fail(QW_ESTATE, "qw_step before qw_set_state");
     if (n == 0) return QW_OK;
-    const bool allow_fast = s->sched != QW_SCHED_GENERIC;
-    s->last_sched = allow_fast ? QW_SCHED_FUSED : QW_SCHED_GENERIC;
-    s->last_k = 1;
-    for (int64_t i = 0; i < n; ++i) {
+    // ---- schedule dispatch (all schedules produce bit-identical states) ----------------------------
+    int sched = s->sched;
+    if (sched == QW_SCHED_AUTO)
+        sched = resident1d_eligible(s) ? QW_SCHED_RESIDENT
+              : (blocked1d_eligible(s) && n >= blocked1d_granule(s)) ? QW_SCHED_BLOCKED : QW_SCHED_FUSED;
+    if (sched == QW_SCHED_RESIDENT) {
+        if (!resident1d_eligible(s))
+            return fail(QW_EUNSUPPORTED, "the resident schedule needs 1D walks of at most 4096 sites, no per-site matrices, no link mask");
+        int rc = launch_step_resident1d(s, s->buf[s->cur], s->buf[1 - s->cur], n);
+        if (rc) return rc;
+        s->cur ^= 1; s->t += n; s->radius += n;
+        s->last_sched = sched; s->last_k = (int)(n > 0x7fffffff ? 0x7fffffff : n);
+        return QW_OK;
+    }
+    if (sched == QW_SCHED_BLOCKED && !blocked1d_eligible(s))
+        return fail(QW_EUNSUPPORTED, "the temporally blocked schedule needs a 1D lattice of >= %d sites with a uniform coin",
+                    32 * blocked1d_granule(s));
+    int64_t remaining = n;
+    s->last_sched = sched; s->last_k = 1;
+    if (sched == QW_SCHED_BLOCKED) {
+        const int M = blocked1d_granule(s);
+        int kmax = s->sched_k > 0 ? s->sched_k : 48;     // measured optimum on B200 (profiles/r01_blocked1d.md)
+        if (kmax > blocked1d_max_k(s)) kmax = blocked1d_max_k(s);
+        kmax = kmax / M * M;
+        if (kmax < M) kmax = M;
+        s->last_k = kmax;
+        while (remaining >= M) {
+            const int kk = (int)(remaining >= kmax ? kmax : remaining / M * M);
+            int rc = launch_step_blocked1d(s, s->buf[s->cur], s->buf[1 - s->cur], kk);
+            if (rc) return rc;
+            s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;
+        }
+    }
+    const bool allow_fast = sched != QW_SCHED_GENERIC;
+    for (int64_t i = 0; i < remaining; ++i) {
         const Box box = step_box(s);
         int rc = launch_step(s, s->buf[s->cur], s->buf[1 - s->cur], box, allow_fast);
         if (rc) return rc;
@@ -415,8 +446,6 @@ int qw_set_schedule(qw_sim *s, int schedule, int k) {
     if (!s) return fail(QW_EINVAL, "handle is NULL");
     if (schedule < QW_SCHED_AUTO || schedule > QW_SCHED_RESIDENT) return fail(QW_EINVAL, "unknown schedule %d", schedule);
     if (k < 0) return fail(QW_EINVAL, "k must be >= 0");
-    if (schedule == QW_SCHED_BLOCKED || schedule == QW_SCHED_RESIDENT)
-        return fail(QW_EUNSUPPORTED, "schedule %d is not available for this configuration", schedule);
     s->sched = schedule; s->sched_k = k;
     return QW_OK;
 }

@@ -64,12 +64,14 @@ template <typename R> __device__ __forceinline__ cplx<R> cx_mulni(cplx<R> a) { r
 template <typename R, int CD, int KIND>
 __device__ __forceinline__ void apply_coin(const R *__restrict__ C, cplx<R> (&v)[CD]) {
     if constexpr (KIND == COIN_HADAMARD && CD == 2) {
-        // s*[[1,1],[1,-1]]: 4 add/sub + 4 mul
+        // s*[[1,1],[1,-1]] as t = s*L; phi_R = s*R + t; phi_L = s*R - t: 2 mul + 4 fma per site
         const R s = C[0];
-        cplx<R> p = cx_add(v[0], v[1]);
-        cplx<R> m = cx_sub(v[0], v[1]);
-        v[0] = cx_scale(s, p);
-        v[1] = cx_scale(s, m);
+        const R tre = mul_rn(s, v[1].re), tim = mul_rn(s, v[1].im);
+        const R are = v[0].re, aim = v[0].im;
+        v[0].re = fma_rn(s, are, tre);
+        v[0].im = fma_rn(s, aim, tim);
+        v[1].re = fma_rn(s, are, -tre);
+        v[1].im = fma_rn(s, aim, -tim);
     } else if constexpr (KIND == COIN_GROVER4 && CD == 4) {
         // off-diagonal g, diagonal d (Grover: g = 1/2, d = -1/2): phi_a = g*sum + (d-g)*psi_a
         const R g = C[2], dg = sub_rn(C[0], C[2]);

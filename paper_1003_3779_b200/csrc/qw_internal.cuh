@@ -118,6 +118,16 @@ int launch_delta(qw_sim *s, const long long *site, const double *coin_vec);
 int launch_step(qw_sim *s, const void *in, void *out, const Box &box, bool allow_fast);
 int launch_step_inverse(qw_sim *s, const void *in, void *out);
 
+// qw_step_blocked1d.cu : k steps per launch, warp-private register tiles (uniform coin, 1D)
+bool blocked1d_eligible(const qw_sim *s);
+int blocked1d_granule(const qw_sim *s);
+int blocked1d_max_k(const qw_sim *s);
+int launch_step_blocked1d(qw_sim *s, const void *in, void *out, int k);
+
+// qw_step_resident1d.cu : one CTA per walk, all n steps on the SM (1D walks of <= 4096 sites)
+bool resident1d_eligible(const qw_sim *s);
+int launch_step_resident1d(qw_sim *s, const void *in, void *out, long long n);
+
 // qw_reduce.cu
 int launch_probabilities(qw_sim *s, const void *state, void *out_dev);
 int launch_moments(qw_sim *s, const void *state, double *out_dev);

@@ -1,0 +1,263 @@
+// qw_step_resident1d.cu — SM-resident 1D walks: one CTA per walk keeps the whole state in registers
+// for ALL n steps of a qw_step call, so HBM is touched only at the start and at the end
+// (BASELINE.json:configs[0] and [4]).
+//
+// Thread `tid` owns the M consecutive sites tid*M .. tid*M+M-1 of both coin planes.  As in the
+// temporally blocked kernel the shift of PAPER.md:46 eq. 3 is a renaming of registers inside a
+// lane (at step s logical site i lives in Rp[(i - s) mod M], Lp[(i + s) mod M]); the one element per
+// plane that crosses a lane boundary travels by warp shuffle, the one per warp that crosses a warp
+// boundary through a double-buffered shared-memory slot (one __syncthreads per step).
+// Per-walk coins C_w (the coin family may differ per walk) are read once into
+// registers; per-site phases e^{i phi_x} (BASELINE.json:configs[4]) live in shared memory.
+// Light cone: a warp whose 32*M sites cannot have been reached yet holds exact
+// zeros and skips its coin arithmetic.
+#include "qw_coin.cuh"
+
+namespace qw {
+
+constexpr int RES_M = 8;             // sites per thread
+constexpr int RES_MAX_THREADS = 512; // -> walks of up to 4096 sites
+constexpr int RES_SMALL_THREADS = 320;
+
+template <typename R>
+struct Resident1dArgs {
+    const typename Cx<R>::T *in;
+    typename Cx<R>::T *out;
+    long long n_sites, walk_stride, plane_stride;
+    long long n_steps;
+    const typename Cx<R>::T *coins;    // per-walk matrices or nullptr (uniform)
+    const typename Cx<R>::T *phases;   // [walk][site] or nullptr
+    int window;                        // 1: skip warps outside the light cone
+    long long centre, radius0;
+    R coin[8];
+};
+
+template <typename R>
+struct ResidentCtx {
+    typename Cx<R>::T *edgeR, *edgeL, *wrapR, *wrapL;   // [2][nw], [2][nw], [2], [2]
+    const typename Cx<R>::T *ph;                        // padded per-site phases of this walk (shared)
+    int lane, wid, nw, tid;
+    bool lo_thread;        // owns site 0
+    int hi_index;          // logical index of site N-1 inside this thread, or -1
+    bool hi_warp;          // some lane of this warp owns site N-1
+    long long warp_lo, warp_hi;   // first / last site of this warp's tile
+    int window;
+    long long centre, radius0;
+};
+
+template <typename R> __device__ __forceinline__ cplx<R> shfl_up_cx(cplx<R> v) {
+    v.re = __shfl_up_sync(0xffffffffu, v.re, 1);
+    v.im = __shfl_up_sync(0xffffffffu, v.im, 1);
+    return v;
+}
+template <typename R> __device__ __forceinline__ cplx<R> shfl_down_cx(cplx<R> v) {
+    v.re = __shfl_down_sync(0xffffffffu, v.re, 1);
+    v.im = __shfl_down_sync(0xffffffffu, v.im, 1);
+    return v;
+}
+template <typename R> __device__ __forceinline__ typename Cx<R>::T to_v(cplx<R> z) {
+    typename Cx<R>::T v; v.x = z.re; v.y = z.im; return v;
+}
+template <typename R> __device__ __forceinline__ cplx<R> from_v(typename Cx<R>::T v) { return cplx<R>{v.x, v.y}; }
+
+// One walk step; U = (steps done so far) mod M, s = steps done so far in this launch.
+template <typename R, int M, int KIND, bool PHASES, bool OPEN, int U>
+__device__ __forceinline__ void resident_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
+                                              const ResidentCtx<R> &cx, long long s) {
+    bool active = true;
+    if (cx.window) {
+        const long long r = cx.radius0 + s + 1;
+        active = (cx.warp_lo <= cx.centre + r) && (cx.warp_hi >= cx.centre - r);
+    }
+    if (active) {
+#pragma unroll
+        for (int i = 0; i < M; ++i) {
+            const int q = (i - U + M) % M, p = (i + U) % M;
+            cplx<R> v[2] = {Rp[q], Lp[p]};
+            apply_coin<R, 2, KIND>(C, v);
+            if constexpr (PHASES) {
+                const cplx<R> ph = from_v<R>(cx.ph[cx.tid * (M + 1) + i]);
+                v[0] = cx_mul(ph.re, ph.im, v[0]);
+                v[1] = cx_mul(ph.re, ph.im, v[1]);
+            }
+            Rp[q] = v[0];
+            Lp[p] = v[1];
+        }
+    }
+    constexpr int QS = (M - 1 - U + M) % M;   // phi_R of logical M-1 -> becomes R' of logical 0
+    constexpr int PS = U % M;                 // phi_L of logical 0   -> becomes L' of logical M-1
+    const cplx<R> outR = Rp[QS], outL = Lp[PS];
+    cplx<R> hiR = {0, 0};                     // phi_R of site N-1 (needed by the wall / the wrap)
+    if (cx.hi_warp) {
+#pragma unroll
+        for (int i = 0; i < M; ++i)
+            if (i == cx.hi_index) hiR = Rp[(i - U + M) % M];
+    }
+    cplx<R> inR = shfl_up_cx(outR), inL = shfl_down_cx(outL);
+    const int par = (int)(s & 1);
+    if (cx.nw > 1) {
+        if (cx.lane == 31) cx.edgeR[par * cx.nw + cx.wid] = to_v<R>(outR);
+        if (cx.lane == 0) cx.edgeL[par * cx.nw + cx.wid] = to_v<R>(outL);
+    }
+    if constexpr (!OPEN) {
+        if (cx.hi_index >= 0) cx.wrapR[par] = to_v<R>(hiR);
+        if (cx.lo_thread) cx.wrapL[par] = to_v<R>(outL);
+    }
+    if (cx.nw > 1) __syncthreads(); else __syncwarp();
+    if (cx.nw > 1) {
+        if (cx.lane == 0 && cx.wid > 0) inR = from_v<R>(cx.edgeR[par * cx.nw + cx.wid - 1]);
+        if (cx.lane == 31 && cx.wid < cx.nw - 1) inL = from_v<R>(cx.edgeL[par * cx.nw + cx.wid + 1]);
+    }
+    Rp[QS] = inR;
+    Lp[PS] = inL;
+    // site 0 and site N-1: reflecting walls (RBL = 0) or the periodic seam
+    if (cx.lo_thread) Rp[QS] = OPEN ? outL : from_v<R>(cx.wrapR[par]);
+    if (cx.hi_warp) {
+        const cplx<R> fix = OPEN ? hiR : from_v<R>(cx.wrapL[par]);
+#pragma unroll
+        for (int i = 0; i < M; ++i)
+            if (i == cx.hi_index) Lp[(i + U + 1) % M] = fix;
+    }
+}
+
+template <typename R, int M, int KIND, bool PHASES, bool OPEN, int U>
+struct ResidentUnroll {
+    static __device__ __forceinline__ void run(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
+                                               const ResidentCtx<R> &cx, long long s, int count) {
+        if (U < count) {
+            resident_step<R, M, KIND, PHASES, OPEN, U>(Rp, Lp, C, cx, s + U);
+            if constexpr (U + 1 < M) ResidentUnroll<R, M, KIND, PHASES, OPEN, U + 1>::run(Rp, Lp, C, cx, s, count);
+        }
+    }
+};
+
+template <typename R, int M, int KIND, bool PHASES, bool OPEN, int MAXT>
+__global__ void __launch_bounds__(MAXT)
+step_resident1d_kernel(const Resident1dArgs<R> a) {
+    typedef typename Cx<R>::T V;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, nw = blockDim.x >> 5;
+    const long long w = blockIdx.x, N = a.n_sites;
+    V *sm = reinterpret_cast<V *>(smem_raw);
+    ResidentCtx<R> cx;
+    cx.edgeR = sm; cx.edgeL = sm + 2 * nw; cx.wrapR = sm + 4 * nw; cx.wrapL = sm + 4 * nw + 2;
+    V *ph = sm + 4 * nw + 4;
+    cx.ph = ph;
+    cx.tid = tid; cx.lane = tid & 31; cx.wid = tid >> 5; cx.nw = nw;
+    const long long x0 = (long long)tid * M;
+    cx.lo_thread = (tid == 0);
+    cx.hi_index = (N - 1 >= x0 && N - 1 < x0 + M) ? (int)(N - 1 - x0) : -1;
+    cx.hi_warp = __any_sync(0xffffffffu, cx.hi_index >= 0);
+    cx.warp_lo = (long long)cx.wid * 32 * M;
+    cx.warp_hi = cx.warp_lo + 32 * M - 1;
+    cx.window = a.window; cx.centre = a.centre; cx.radius0 = a.radius0;
+
+    if constexpr (PHASES) {
+        for (long long e = tid; e < (long long)blockDim.x * M; e += blockDim.x) {
+            V z; z.x = 0; z.y = 0;
+            if (e < N) z = a.phases[w * N + e];
+            ph[(e / M) * (M + 1) + (e % M)] = z;
+        }
+    }
+    R C[8];
+    if (a.coins) {
+        const R *Cg = reinterpret_cast<const R *>(a.coins + w * 4);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) C[i] = Cg[i];
+    } else {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) C[i] = a.coin[i];
+    }
+    cplx<R> Rp[M], Lp[M];
+    const V *inw = a.in + w * a.walk_stride;
+#pragma unroll
+    for (int i = 0; i < M; ++i) {
+        V r, l; r.x = r.y = 0; l.x = l.y = 0;
+        if (x0 + i < N) { r = inw[x0 + i]; l = inw[a.plane_stride + x0 + i]; }
+        Rp[i] = from_v<R>(r); Lp[i] = from_v<R>(l);
+    }
+    __syncthreads();
+
+    long long s = 0;
+    for (; s + M <= a.n_steps; s += M)
+        ResidentUnroll<R, M, KIND, PHASES, OPEN, 0>::run(Rp, Lp, C, cx, s, M);
+    const int rem = (int)(a.n_steps - s);
+    if (rem > 0) {
+        ResidentUnroll<R, M, KIND, PHASES, OPEN, 0>::run(Rp, Lp, C, cx, s, rem);
+        // undo the register renaming of the last `rem` steps: logical i sits in Rp[(i-rem)%M], Lp[(i+rem)%M]
+        for (int j = 0; j < rem; ++j) {
+            const cplx<R> tr = Rp[M - 1], tl = Lp[0];
+#pragma unroll
+            for (int i = M - 1; i > 0; --i) Rp[i] = Rp[i - 1];
+            Rp[0] = tr;
+#pragma unroll
+            for (int i = 0; i < M - 1; ++i) Lp[i] = Lp[i + 1];
+            Lp[M - 1] = tl;
+        }
+    }
+    V *outw = a.out + w * a.walk_stride;
+#pragma unroll
+    for (int i = 0; i < M; ++i) {
+        if (x0 + i < N) { outw[x0 + i] = to_v<R>(Rp[i]); outw[a.plane_stride + x0 + i] = to_v<R>(Lp[i]); }
+    }
+}
+
+bool resident1d_eligible(const qw_sim *s) {
+    const Geom &g = s->g;
+    return g.dim == 1 && g.en <= (long long)RES_MAX_THREADS * RES_M && s->coin_mode != QW_COIN_PER_SITE &&
+           !s->d_broken && g.batch <= 0x7fffffffLL;
+}
+
+template <typename R, int KIND, bool PHASES>
+static int launch_resident_t(qw_sim *s, const void *in, void *out, long long n) {
+    typedef typename Cx<R>::T V;
+    const Geom &g = s->g;
+    Resident1dArgs<R> a;
+    a.in = static_cast<const V *>(in); a.out = static_cast<V *>(out);
+    a.n_sites = g.en; a.walk_stride = g.walk_stride; a.plane_stride = g.plane_stride; a.n_steps = n;
+    a.coins = s->coin_mode == QW_COIN_PER_WALK ? static_cast<const V *>(s->d_coin) : nullptr;
+    a.phases = static_cast<const V *>(s->d_phases);
+    // the cone test is only meaningful while the cone has not wrapped around a periodic lattice
+    const bool cone_ok = s->window_enabled && s->window_valid &&
+                         (g.boundary == QW_OPEN || (s->centre[0] - (s->radius + n + 1) >= 0 && s->centre[0] + (s->radius + n + 1) < g.en));
+    a.window = cone_ok ? 1 : 0; a.centre = s->centre[0]; a.radius0 = s->radius;
+    for (int i = 0; i < 8; ++i) a.coin[i] = (R)s->h_coin[i];
+    int threads = (int)((g.en + RES_M - 1) / RES_M);
+    threads = (threads + 31) / 32 * 32;
+    const int nw = threads / 32;
+    const size_t smem = sizeof(V) * (size_t)(4 * nw + 4 + (PHASES ? (size_t)threads * (RES_M + 1) : 0));
+    auto launch = [&](auto kernel) -> int {
+        if (smem > 48 * 1024)
+            QW_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kernel<<<(unsigned)g.batch, threads, smem, s->stream>>>(a);
+        return QW_OK;
+    };
+    // two register budgets: walks of <= 320*M sites may use up to 204 registers per thread
+    int rc;
+    if (threads <= RES_SMALL_THREADS)
+        rc = g.boundary == QW_OPEN ? launch(step_resident1d_kernel<R, RES_M, KIND, PHASES, true, RES_SMALL_THREADS>)
+                                   : launch(step_resident1d_kernel<R, RES_M, KIND, PHASES, false, RES_SMALL_THREADS>);
+    else
+        rc = g.boundary == QW_OPEN ? launch(step_resident1d_kernel<R, RES_M, KIND, PHASES, true, RES_MAX_THREADS>)
+                                   : launch(step_resident1d_kernel<R, RES_M, KIND, PHASES, false, RES_MAX_THREADS>);
+    if (rc) return rc;
+    QW_LAUNCH_CHECK(s, "step_resident1d_kernel");
+    return QW_OK;
+}
+
+int launch_step_resident1d(qw_sim *s, const void *in, void *out, long long n) {
+    const bool had = s->coin_mode == QW_COIN_UNIFORM && s->coin_kind == COIN_HADAMARD;
+    const bool ph = s->d_phases != nullptr;
+    if (s->dtype == QW_C128) {
+        if (had) return ph ? launch_resident_t<double, COIN_HADAMARD, true>(s, in, out, n)
+                           : launch_resident_t<double, COIN_HADAMARD, false>(s, in, out, n);
+        return ph ? launch_resident_t<double, COIN_GENERAL, true>(s, in, out, n)
+                  : launch_resident_t<double, COIN_GENERAL, false>(s, in, out, n);
+    }
+    if (had) return ph ? launch_resident_t<float, COIN_HADAMARD, true>(s, in, out, n)
+                       : launch_resident_t<float, COIN_HADAMARD, false>(s, in, out, n);
+    return ph ? launch_resident_t<float, COIN_GENERAL, true>(s, in, out, n)
+              : launch_resident_t<float, COIN_GENERAL, false>(s, in, out, n);
+}
+
+}  // namespace qw

@@ -213,6 +213,88 @@ def test_generic_and_fused_schedules_agree_bit_for_bit(qw, dev):
         assert np.array_equal(a[0], b[0]), w.name
 
 
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.PERIODIC, qi.OPEN])
+@pytest.mark.parametrize("coin", ["hadamard", "su2"])
+def test_blocked_1d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, dtype, boundary, coin, ):
+    """P13: k steps per HBM round trip (warp-private register tiles) == k fused single steps, bit for bit;
+    sizes span several tiles, a ragged last tile and the periodic seam / the reflecting walls."""
+    rng = np.random.default_rng(3)
+    for sites, steps, k, batch in ((5000, 96, 32, 1), (1031, 100, 16, 3), (70001, 131, 0, 1), (512, 48, 48, 2)):
+        c = qi.hadamard(dtype) if coin == "hadamard" else qi.su2(*rng.uniform(0, 2 * np.pi, 3)).astype(dtype)
+        w = qi.Workload("blk", 1, (sites,), batch, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
+                        state=qi.random_state(9, batch, sites, 2, dtype, normalise_per_walk=True))
+        a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_BLOCKED, k=k)
+        assert b[3]["sched"] == qw.QW_SCHED_BLOCKED and b[3]["launches"] < a[3]["launches"]
+        assert np.array_equal(a[0], b[0]), (sites, steps, k)
+        auto = gpu_run(qw, w)
+        assert np.array_equal(a[0], auto[0])
+    check_parity(w, b, oracle_run(oracle, w))
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.PERIODIC, qi.OPEN])
+def test_resident_1d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, dtype, boundary):
+    """P13: one CTA per walk with the state in registers for all n steps == n fused single steps."""
+    rng = np.random.default_rng(4)
+    for sites, steps, batch, kind in ((1, 5, 2, "su2"), (2, 7, 2, "had"), (3, 9, 1, "su2"), (37, 100, 3, "had"),
+                                      (201, 131, 2, "su2+ph"), (256, 64, 1, "had"), (257, 33, 2, "perwalk+ph"),
+                                      (2049, 75, 3, "perwalk+ph"), (4096, 41, 2, "had"), (4095, 18, 1, "perwalk")):
+        if kind.startswith("perwalk"):
+            a3 = rng.uniform(0, 2 * np.pi, (batch, 3))
+            mode, c = qi.COIN_PER_WALK, qi.su2(a3[:, 0], a3[:, 1], a3[:, 2]).astype(dtype)
+        elif kind.startswith("su2"):
+            mode, c = qi.COIN_UNIFORM, qi.su2(*rng.uniform(0, 2 * np.pi, 3)).astype(dtype)
+        else:
+            mode, c = qi.COIN_UNIFORM, qi.hadamard(dtype)
+        ph = np.exp(1j * rng.uniform(0, 2 * np.pi, (batch, sites))).astype(dtype) if kind.endswith("+ph") else None
+        w = qi.Workload("res", 1, (sites,), batch, boundary, np.dtype(dtype), steps, mode, c, phases=ph,
+                        state=qi.random_state(19, batch, sites, 2, dtype, normalise_per_walk=True))
+        a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_RESIDENT)
+        assert b[3]["sched"] == qw.QW_SCHED_RESIDENT and b[3]["launches"] < a[3]["launches"]
+        assert np.array_equal(a[0], b[0]), (sites, steps, kind)
+        auto = gpu_run(qw, w)
+        assert auto[3]["sched"] == qw.QW_SCHED_RESIDENT and np.array_equal(a[0], auto[0])
+        check_parity(w, b, oracle_run(oracle, w))
+
+
+@pytest.mark.parametrize("window", [True, False])
+def test_resident_delta_start_with_light_cone(qw, oracle, dev, window):
+    for w in (qi.k0(steps=130), qi.k4(batch=6, half=300, steps=450), qi.k4(batch=2, half=1024, steps=1024)):
+        a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_RESIDENT, window=window)
+        assert np.array_equal(a[0], b[0]), w.name
+        if w.batch <= 2:
+            check_parity(w, b, oracle_run(oracle, w))
+    # split stepping: two resident launches continue the same cone
+    w = qi.k4(batch=3, half=200, steps=150)
+    h = qw.create_for(w)
+    try:
+        qw.qw_set_window(h, window)
+        qw.load_state(h, w)
+        qw.qw_step(h, 70); qw.qw_step(h, 80)
+        got = np.empty((w.batch, w.sites, 2), dtype=w.dtype)
+        qw.qw_get_state(h, got)
+    finally:
+        qw.qw_destroy(h)
+    assert np.array_equal(got, gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)[0])
+
+
+def test_blocked_schedule_rejected_where_it_does_not_apply(qw, dev):
+    w = qi.k3(extents=(64, 64), steps=4, coin="dft")
+    h = qw.create_for(w)
+    try:
+        qw.load_state(h, w)
+        qw.qw_set_schedule(h, qw.QW_SCHED_BLOCKED, 0)
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_step(h, 4)
+        assert ei.value.code == qw.QW_EUNSUPPORTED
+    finally:
+        qw.qw_destroy(h)
+
+
 @pytest.mark.parametrize("wl", ["k0", "k2", "k4", "k2-periodic-corner"])
 def test_light_cone_window_is_exact(qw, dev, wl):
     """the 'line' variant updates only the sites the walker can have reached."""
