@@ -76,6 +76,33 @@ def workload_config(name, w, extra=None):
     return cfg
 
 
+def coin_cost(w):
+    """(instructions, flops) per site-step of csrc/qw_coin.cuh::apply_coin for this workload's coin
+    (DESIGN.md section 5): mul = 1 flop, fma = 2 flops, add = 1 flop."""
+    c = np.asarray(w.coin)
+    if w.dim == 1:
+        had = w.coin_mode == qi.COIN_UNIFORM and np.all(c.imag == 0) and c[0, 0] == c[0, 1] == c[1, 0] == -c[1, 1]
+        instr, flops = (6, 10) if had else (16, 28)
+        if w.phases is not None:
+            instr, flops = instr + 8, flops + 12
+        return instr, flops
+    if w.coin_mode == qi.COIN_UNIFORM and np.all(c.imag == 0) and np.all(np.abs(c) == abs(c[0, 0])):
+        if np.array_equal(np.sign(c.real), np.sign(qi.hadamard_x_hadamard().real)):
+            return 24, 24
+    if w.coin_mode == qi.COIN_UNIFORM and np.array_equal(c, qi.grover4(c.dtype)):
+        return 16, 24
+    if w.coin_mode == qi.COIN_UNIFORM and np.array_equal(c, qi.dft4(c.dtype)):
+        return 24, 24
+    return 64, 120
+
+
+def alu_peak(w, sm_max_mhz):
+    """Plain-ALU peak: 148 SMs x 64 FP64 (128 FP32) FMA lanes x SM clock (B200)."""
+    lanes = 64 if w.dtype == np.complex128 else 128
+    ghz = (sm_max_mhz or 1965.0) / 1e3
+    return 148 * lanes * ghz * 1e9      # instructions/s; x2 for FMA flops
+
+
 def measured_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -407,28 +434,64 @@ def run_gpu(args):
         e_val, e_ms = aggregate_rate(site_updates_per_step * n_e2e, e2e_ms, world, dev)
         e2e = {"value": e_val, "unit": METRIC, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": e_ms / n_e2e, "steps": n_e2e, "api": "qw_set_state(host) + qw_step + qw_moments/qw_probabilities(host)"}
+    # ---- single-step leg: the fused coin+shift kernel alone (HBM roofline evidence) -----------
+    fused = None
+    if sched != qw.QW_SCHED_FUSED and not args.no_fused_leg:
+        nf = min(w.steps, 100)
+        qw.qw_set_schedule(h, qw.QW_SCHED_FUSED, 0)
+        qw.qw_set_window(h, 0)
+        if delta:   # leave the delta neighbourhood: a spread-out state, full-lattice launches
+            qw.qw_set_state_delta(h, w.delta_site, delta_coin)
+        qw.qw_step(h, 3)
+        torch.cuda.synchronize(); barrier(world)
+        fa = torch.cuda.Event(enable_timing=True); fb = torch.cuda.Event(enable_timing=True)
+        fa.record(stream)
+        qw.qw_step(h, nf)
+        fb.record(stream)
+        torch.cuda.synchronize()
+        fms = max_over_ranks(fa.elapsed_time(fb), world, dev)
+        fused = {"walk_steps": nf, "avg_launch_ms": fms / nf,
+                 "site_updates_per_s": float(w.sites) * w.batch * nf / (fms * 1e-3)}
     qw.qw_destroy(h)
 
     if rank != 0:
         return 0
     peak, peak_src = measured_peak()
-    n_step_launches = w.steps * args.steps if kdepth <= 1 else None
-    kernel_ms = step_ms / args.steps            # device time of qw_step(walk_steps), gaps included
+    kernel_ms = step_ms / args.steps            # device time of the hot path per bench step, gaps included
     eff_gbs = site_updates_per_step * alg_bytes_per_site / (kernel_ms * 1e-3) / 1e9
     sched_name = {0: "auto", 1: "generic", 2: "fused", 3: "blocked", 4: "resident"}.get(sched, str(sched))
-    roofline = {
-        "bound": "hbm" if sched in (1, 2) else "alu",
-        "kernel": {1: "step_scatter_kernel (generic)", 2: "step_scatter_kernel (fused coin+shift)",
-                   3: "step_blocked_kernel", 4: "step_resident_kernel"}.get(sched, "?"),
-        "achieved": eff_gbs, "peak": peak, "unit": "GB/s", "frac": eff_gbs / peak,
-        "peak_source": "of " + peak_src,
-        "frac_of_nominal_8000": eff_gbs / 8000.0,
-        "algorithmic_bytes_per_site_step": alg_bytes_per_site,
-        "avg_launch_ms": (step_ms / (w.steps * args.steps)) if kdepth <= 1 else None,
-        "traffic": stored_traffic(args.workload),
-        "note": "achieved = 2*coin_dim*sizeof(complex) bytes x site-updates / CUDA-event time of qw_step; "
-                "for blocked/resident schedules this is the EFFECTIVE bandwidth (may exceed the HBM peak)",
-    }
+    kname = {1: "step_scatter_kernel (generic)", 2: "step_scatter_kernel (fused coin+shift)",
+             3: "step_blocked1d_kernel", 4: "step_resident1d_kernel"}.get(sched, "?")
+    if sched in (1, 2):
+        roofline = {
+            "bound": "hbm", "kernel": kname, "achieved": eff_gbs, "peak": peak, "unit": "GB/s", "frac": eff_gbs / peak,
+            "peak_source": "of " + peak_src, "frac_of_nominal_8000": eff_gbs / 8000.0,
+            "algorithmic_bytes_per_site_step": alg_bytes_per_site,
+            "avg_launch_ms": step_ms / (w.steps * args.steps),
+            "traffic": stored_traffic(args.workload),
+            "note": "achieved = 2*coin_dim*sizeof(complex) B x site-updates / CUDA-event time of qw_step (launch gaps included)"
+                    + ("; light-cone window active: site-updates are counted on the FULL lattice, so this is an effective figure" if windowed else ""),
+        }
+    else:
+        instr, flops = coin_cost(w)
+        ipeak = alu_peak(w, clocks["sm_max_mhz"] if clocks else None)
+        rate = site_updates_per_step / (kernel_ms * 1e-3)
+        roofline = {
+            "bound": "alu", "kernel": kname, "achieved": rate * flops / 1e12, "peak": 2 * ipeak / 1e12, "unit": "TFLOP/s",
+            "frac": rate * flops / (2 * ipeak), "instr_issue_frac": rate * instr / ipeak,
+            "peak_source": "derived: 148 SMs x %d %s FMA lanes x sm_max_mhz x 2 (DESIGN.md section 5)"
+                           % (64 if w.dtype == np.complex128 else 128, "FP64" if w.dtype == np.complex128 else "FP32"),
+            "algorithmic_flops_per_site_step": flops, "algorithmic_instr_per_site_step": instr,
+            "traffic": stored_traffic(args.workload + "_" + sched_name),
+            "effective_hbm_gbs_vs_single_step": eff_gbs, "single_step_hbm_roofline_x": eff_gbs / peak,
+            "note": "temporal blocking / SM residency removes the HBM bound; algorithmic flops exclude halo recomputation"
+                    + ("; light-cone window active: counted on the FULL lattice (effective)" if windowed else ""),
+        }
+    if fused is not None:
+        fg = fused["site_updates_per_s"] * alg_bytes_per_site / 1e9
+        fused.update({"bound": "hbm", "kernel": "step_scatter_kernel (fused coin+shift)", "achieved": fg, "peak": peak,
+                      "unit": "GB/s", "frac": fg / peak, "frac_of_nominal_8000": fg / 8000.0,
+                      "traffic": stored_traffic(args.workload)})
     line = {
         "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -438,6 +501,7 @@ def run_gpu(args):
                                                      "step_ms": step_ms / args.steps, "outputs_ms": out_ms / args.steps}),
         "effective_hbm_gbs": eff_gbs,
         "roofline": roofline,
+        "fused_single_step": fused,
         "clocks": clocks,
         "gpu_launches": int(launches),
         "e2e": e2e,
@@ -463,6 +527,7 @@ def main():
     ap.add_argument("--k", type=int, default=0)
     ap.add_argument("--no-window", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-fused-leg", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

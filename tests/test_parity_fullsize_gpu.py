@@ -1,0 +1,194 @@
+"""Full-size parity: the five BASELINE.json configs at their real sizes, in the launch configuration
+bench.py times (schedule AUTO, light-cone window on), checked against the oracle on SAMPLED outputs it
+can compute one by one:
+
+  * an amplitude at site x after t steps depends only on the initial state inside the light cone
+    [x - t, x + t] (eq. 15 :160, eq. 18 :210), so the oracle evolves just that window
+    (open ends, far enough away) and the centre sites must agree to the usual gates;
+  * the reductions (qw_moments / qw_probabilities) are checked against the oracle's reductions applied to
+    the state the GPU produced (same input bytes), plus the invariants that hold at any size.
+"""
+import numpy as np
+import pytest
+
+from paper_1003_3779_b200 import inputs as qi
+
+pytestmark = pytest.mark.gpu
+
+AMP_TOL = {np.dtype(np.complex128): 1e-12, np.dtype(np.complex64): 2e-5}
+
+
+@pytest.fixture(scope="module")
+def dev(qw):
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch.device("cuda:0")
+
+
+def run_full(qw, w, steps=None):
+    """-> (AoS final state on the host, moments, info)"""
+    h = qw.create_for(w)
+    try:
+        qw.load_state(h, w)
+        qw.qw_step(h, w.steps if steps is None else steps)
+        out = np.empty((w.batch, w.sites, w.coin_dim), dtype=w.dtype)
+        qw.qw_get_state(h, out)
+        mom = np.empty((w.batch, 3 if w.dim == 1 else 6))
+        qw.qw_moments(h, mom)
+        P = np.empty((w.batch, w.sites), dtype=np.float64 if w.dtype == np.complex128 else np.float32)
+        qw.qw_probabilities(h, P)
+        info = {"sched": qw.qw_get_info(h, qw.QW_INFO_LAST_SCHEDULE), "k": qw.qw_get_info(h, qw.QW_INFO_LAST_K),
+                "launches": qw.qw_get_info(h, qw.QW_INFO_LAUNCHES)}
+    finally:
+        qw.qw_destroy(h)
+    return out, mom, P, info
+
+
+def check_reductions(oracle, w, final, mom, P, rtol):
+    """Oracle reductions on the very state the GPU holds (promoted to double)."""
+    st = np.ascontiguousarray(final.astype(np.complex128))
+    momo = oracle.moments(w.extents, st, batch=w.batch)
+    Po = oracle.probabilities(w.extents, st, batch=w.batch)
+    ptol = 1e-12 if w.dtype == np.complex128 else 1e-6 * float(Po.max()) + 1e-12
+    assert np.max(np.abs(P.astype(np.float64) - Po)) <= ptol
+    nm = 1 if w.dim == 1 else 2
+    ext = max(w.extents)
+    for b in range(0, w.batch, max(1, w.batch // 64)):
+        assert abs(mom[b, 0] - momo[b, 0]) <= rtol * momo[b, 0]
+        for j in range(1, 1 + nm):
+            assert abs(mom[b, j] - momo[b, j]) <= rtol * (abs(momo[b, j]) + ext)
+        second = 1.0 + max(abs(momo[b, j]) for j in range(1 + nm, mom.shape[1])) + max(momo[b, j] ** 2 for j in range(1, 1 + nm))
+        for j in range(1 + nm, mom.shape[1]):
+            assert abs(mom[b, j] - momo[b, j]) <= rtol * second
+
+
+# ------------------------------------------------------------------ K1: ring of 2^26 sites, 1000 steps
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+def test_k1_full_size_sampled_light_cones(qw, oracle, dev, dtype):
+    w = qi.k1(dtype=dtype)
+    N, t = w.sites, w.steps
+    final, mom, P, info = run_full(qw, w)
+    assert info["sched"] == qw.QW_SCHED_BLOCKED            # the configuration bench.py times
+    init = w.state[0]
+    rng = np.random.default_rng(1)
+    # seam, tile edges of the blocked kernel (valid = 512 - 2k sites per warp tile), random sites
+    valid = 512 - 2 * info["k"]
+    centres = [0, 5, N - 3, N // 2, valid, valid - 1, 7 * valid + 1, 4 * valid * 1000, N - valid] + \
+        [int(x) for x in rng.integers(0, N, 23)]
+    pad = 8
+    half = t + pad
+    worst = 0.0
+    coin = w.coin.astype(np.complex128)
+    for c in centres:
+        idx = (np.arange(c - half, c + half + 1) % N)
+        win = np.ascontiguousarray(init[idx].astype(np.complex128))[None]
+        oracle.step((2 * half + 1,), coin, win, t, boundary=qi.OPEN)
+        got = final[0, idx[half - pad:half + pad + 1]].astype(np.complex128)
+        want = win[0, half - pad:half + pad + 1]
+        worst = max(worst, float(np.max(np.abs(got - want))))
+    assert worst <= AMP_TOL[np.dtype(dtype)], worst
+    # invariants + reductions at full size
+    if dtype == np.complex128:
+        assert abs(mom[0, 0] - 1) <= 1e-14 + 2e-16 * t + 1e-12        # R23 drift (+ summation slack)
+    else:
+        assert abs(mom[0, 0] - 1) <= 1e-4
+    check_reductions(oracle, w, final, mom, P, 1e-10 if dtype == np.complex128 else 1e-4)
+
+
+# ------------------------------------------------------------------ K3: torus 8192^2, complex64
+@pytest.mark.parametrize("coin,steps,nsamples", [("hxh", 96, 6), ("dft", 96, 6), ("dft", 500, 1)])
+def test_k3_full_size_sampled_light_cones(qw, oracle, dev, coin, steps, nsamples):
+    w = qi.k3(coin=coin, steps=steps)
+    E = w.extents[0]
+    final, mom, P, info = run_full(qw, w)
+    init = w.state[0].reshape(E, E, 4)
+    fin = final[0].reshape(E, E, 4)
+    rng = np.random.default_rng(2)
+    centres = [(0, 0), (E - 1, 17), (E // 2, E - 1), (4095, 4096)][:nsamples] + \
+        [tuple(int(v) for v in rng.integers(0, E, 2)) for _ in range(max(0, nsamples - 4))]
+    pad = 2
+    half = steps + pad
+    c128 = w.coin.astype(np.complex128)
+    worst = 0.0
+    for (cm, cn) in centres:
+        im = np.arange(cm - half, cm + half + 1) % E
+        inn = np.arange(cn - half, cn + half + 1) % E
+        win = np.ascontiguousarray(init[np.ix_(im, inn)].astype(np.complex128)).reshape(1, -1, 4)
+        side = 2 * half + 1
+        oracle.step((side, side), c128, win, steps, boundary=qi.OPEN)
+        want = win.reshape(side, side, 4)[half - pad:half + pad + 1, half - pad:half + pad + 1]
+        got = fin[np.ix_(im[half - pad:half + pad + 1], inn[half - pad:half + pad + 1])].astype(np.complex128)
+        worst = max(worst, float(np.max(np.abs(got - want))))
+    assert worst <= 2e-5, worst
+    assert abs(mom[0, 0] - 1) <= 1e-4
+    if steps == 96 and coin == "dft":
+        check_reductions(oracle, w, final, mom, P, 1e-4)
+
+
+# ------------------------------------------------------------------ K2: open 4097^2 Grover walk
+def test_k2_full_lattice_300_steps_against_the_whole_light_cone(qw, oracle, dev):
+    """Full 4097^2 lattice, 300 steps: the oracle evolves the whole (2*300+3)^2 support."""
+    steps = 300
+    w = qi.k2(steps=steps)
+    final, mom, P, info = run_full(qw, w)
+    half = steps + 1
+    side = 2 * half + 1
+    wo = qi.k2(half=half, steps=steps)
+    psi = wo.initial_state()
+    oracle.step(wo.extents, wo.coin, psi, steps, boundary=qi.OPEN)
+    fin = final[0].reshape(4097, 4097, 4)
+    c = 2048
+    got = fin[c - half:c + half + 1, c - half:c + half + 1]
+    assert np.max(np.abs(got - psi.reshape(side, side, 4))) <= 1e-12
+    outside = fin.copy()
+    outside[c - half:c + half + 1, c - half:c + half + 1] = 0
+    assert not outside.any()                                   # exact zeros outside the cone
+    Po = oracle.probabilities(wo.extents, psi)[0].reshape(side, side)
+    assert np.max(np.abs(P[0].reshape(4097, 4097)[c - half:c + half + 1, c - half:c + half + 1] - Po)) <= 1e-12
+
+
+def test_k2_full_config_invariants(qw, oracle, dev):
+    """The real config (2048 steps): properties that hold at any size + the oracle's reductions."""
+    w = qi.k2()
+    final, mom, P, info = run_full(qw, w)
+    Pg = P[0].reshape(4097, 4097)
+    assert abs(Pg.sum() - 1) <= 1e-12 and abs(mom[0, 0] - 1) <= 1e-12       # Grover entries are exact: no drift
+    m, n = np.meshgrid(np.arange(-2048, 2049), np.arange(-2048, 2049), indexing="ij", sparse=True)
+    outside = (np.abs(m) + np.abs(n) > 2048) | (((m + n) % 2) == 1)          # diamond, parity of t = 2048
+    assert not Pg[outside].any()
+    assert np.max(np.abs(Pg - Pg[::-1, :])) < 1e-15 and np.max(np.abs(Pg - Pg.T)) < 1e-15
+    assert abs(mom[0, 1]) < 1e-9 and abs(mom[0, 2]) < 1e-9 and abs(mom[0, 5]) < 1e-6
+    check_reductions(oracle, w, final, mom, P, 1e-10)
+
+
+# ------------------------------------------------------------------ K4: 4096 disordered walks
+def test_k4_full_config_sampled_walks(qw, oracle, dev):
+    w = qi.k4()
+    final, mom, P, info = run_full(qw, w)
+    assert info["sched"] == qw.QW_SCHED_RESIDENT and info["launches"] <= 12
+    mode, coin = w.general_coin_f64()
+    pick = [0, 1, 147, 148, 2047, 4095] + [int(x) for x in np.random.default_rng(3).integers(0, 4096, 10)]
+    init = w.initial_state()
+    worst = 0.0
+    for b in pick:
+        psi = np.ascontiguousarray(init[b:b + 1].astype(np.complex128))
+        oracle.step(w.extents, coin[b:b + 1], psi, w.steps, boundary=qi.OPEN, coin_mode=mode)
+        worst = max(worst, float(np.max(np.abs(final[b] - psi[0]))))
+        mo = oracle.moments(w.extents, psi)[0]
+        assert abs(mom[b, 0] - mo[0]) <= 1e-10 and abs(mom[b, 1] - mo[1]) <= 1e-10 * 2049 + 1e-10 * abs(mo[1])
+        assert abs(mom[b, 2] - mo[2]) <= 1e-10 * (1 + abs(mo[2]) + mo[1] ** 2)
+        Po = oracle.probabilities(w.extents, psi)[0]
+        assert np.max(np.abs(P[b] - Po)) <= 1e-12
+    assert worst <= 1e-12, worst
+    assert np.max(np.abs(mom[:, 0] - 1)) <= 1e-12
+
+
+def test_k0_is_the_full_config(qw, oracle, dev):
+    w = qi.k0()
+    final, mom, P, info = run_full(qw, w)
+    psi = w.initial_state()
+    oracle.step(w.extents, w.coin, psi, w.steps, boundary=qi.OPEN)
+    assert np.max(np.abs(final - psi)) <= 1e-12
+    assert np.max(np.abs(P - oracle.probabilities(w.extents, psi))) <= 1e-12
+    assert info["sched"] == qw.QW_SCHED_RESIDENT
