@@ -137,9 +137,11 @@ int qw_create_batch(int64_t batch, int dim, const int64_t *extents, int coin_dim
     s->esize = dtype == QW_C128 ? 16 : 8;
     // row pitch: 128-byte aligned rows when there is more than one row, else 16-byte aligned
     const long long align_elems = ((batch * g.em > 1) ? 128 : 16) / (long long)s->esize;
-    g.pitch = (g.en + align_elems - 1) / align_elems * align_elems;
-    g.walk_stride = g.em * g.pitch;
+    g.ghost = dim == 2 ? QW_GHOST_2D : 0;
+    g.pitch = (g.en + 2 * g.ghost + align_elems - 1) / align_elems * align_elems;
+    g.walk_stride = (g.em + 2 * g.ghost) * g.pitch;
     g.plane_stride = g.batch * g.walk_stride;
+    g.origin = (long long)g.ghost * g.pitch + g.ghost;
     s->device = dev; s->sm_count = sms; s->stream = 0;
     s->state_bytes = (size_t)g.cdim * (size_t)g.plane_stride * s->esize;
     s->window_enabled = true;
@@ -284,8 +286,8 @@ int qw_set_state(qw_sim *s, const void *amps) {
         src = s->scratch;
     }
     s->cur = 0;
-    if (g.pitch != g.en) QW_CUDA(cudaMemsetAsync(s->buf[0], 0, s->state_bytes, s->stream));
-    int rc = launch_aos_to_soa(s, src, s->buf[0]);
+    if (g.pitch != g.en || g.ghost) QW_CUDA(cudaMemsetAsync(s->buf[0], 0, s->state_bytes, s->stream));
+    int rc = launch_aos_to_soa(s, src, state_ptr(s, 0));
     if (rc) return rc;
     if (src == s->scratch) QW_CUDA(cudaStreamSynchronize(s->stream));   // host buffer reusable on return
     s->has_state = true; s->t = 0; s->window_valid = false;
@@ -333,10 +335,10 @@ int qw_get_state(const qw_sim *cs, void *amps) {
     if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
     const Geom &g = s->g;
     const size_t bytes = (size_t)g.batch * (size_t)g.sites * (size_t)g.cdim * s->esize;
-    if (is_device_ptr(amps)) return launch_soa_to_aos(s, s->buf[s->cur], amps);
+    if (is_device_ptr(amps)) return launch_soa_to_aos(s, state_ptr(s, s->cur), amps);
     int rc = ensure_scratch(s, bytes);
     if (rc) return rc;
-    rc = launch_soa_to_aos(s, s->buf[s->cur], s->scratch);
+    rc = launch_soa_to_aos(s, state_ptr(s, s->cur), s->scratch);
     if (rc) return rc;
     QW_CUDA(cudaMemcpyAsync(amps, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
     QW_CUDA(cudaStreamSynchronize(s->stream));
@@ -354,21 +356,35 @@ int qw_step(qw_sim *s, int64_t n) {
     int sched = s->sched;
     if (sched == QW_SCHED_AUTO)
         sched = resident1d_eligible(s) ? QW_SCHED_RESIDENT
-              : (blocked1d_eligible(s) && n >= blocked1d_granule(s)) ? QW_SCHED_BLOCKED : QW_SCHED_FUSED;
+              : (blocked1d_eligible(s) && n >= blocked1d_granule(s)) ? QW_SCHED_BLOCKED
+              : (blocked2d_eligible(s) && n >= 2 && !(s->window_enabled && s->window_valid)) ? QW_SCHED_BLOCKED : QW_SCHED_FUSED;
     if (sched == QW_SCHED_RESIDENT) {
         if (!resident1d_eligible(s))
             return fail(QW_EUNSUPPORTED, "the resident schedule needs 1D walks of at most 4096 sites, no per-site matrices, no link mask");
-        int rc = launch_step_resident1d(s, s->buf[s->cur], s->buf[1 - s->cur], n);
+        int rc = launch_step_resident1d(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), n);
         if (rc) return rc;
         s->cur ^= 1; s->t += n; s->radius += n;
         s->last_sched = sched; s->last_k = (int)(n > 0x7fffffff ? 0x7fffffff : n);
         return QW_OK;
     }
-    if (sched == QW_SCHED_BLOCKED && !blocked1d_eligible(s))
-        return fail(QW_EUNSUPPORTED, "the temporally blocked schedule needs a 1D lattice of >= %d sites with a uniform coin",
+    if (sched == QW_SCHED_BLOCKED && !blocked1d_eligible(s) && !blocked2d_eligible(s))
+        return fail(QW_EUNSUPPORTED, "the temporally blocked schedule needs a uniform coin without phases or link mask on a 1D "
+                                     "lattice of >= %d sites or a natural 2D lattice of >= 32 x 32 sites",
                     32 * blocked1d_granule(s));
     int64_t remaining = n;
     s->last_sched = sched; s->last_k = 1;
+    if (sched == QW_SCHED_BLOCKED && s->g.dim == 2) {
+        int kmax = s->sched_k > 0 ? s->sched_k : (s->dtype == QW_C128 ? 4 : 6);   // measured optima (profiles/)
+        if (kmax > blocked2d_max_k(s)) kmax = blocked2d_max_k(s);
+        s->last_k = kmax;
+        while (remaining > 0) {
+            const int kk = (int)(remaining >= kmax ? kmax : remaining);
+            int rc = launch_step_blocked2d(s, s->cur, 1 - s->cur, kk);
+            if (rc) return rc;
+            s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;
+        }
+        return QW_OK;
+    }
     if (sched == QW_SCHED_BLOCKED) {
         const int M = blocked1d_granule(s);
         int kmax = s->sched_k > 0 ? s->sched_k : 48;     // measured optimum on B200 (profiles/r01_blocked1d.md)
@@ -378,7 +394,7 @@ int qw_step(qw_sim *s, int64_t n) {
         s->last_k = kmax;
         while (remaining >= M) {
             const int kk = (int)(remaining >= kmax ? kmax : remaining / M * M);
-            int rc = launch_step_blocked1d(s, s->buf[s->cur], s->buf[1 - s->cur], kk);
+            int rc = launch_step_blocked1d(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), kk);
             if (rc) return rc;
             s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;
         }
@@ -386,7 +402,7 @@ int qw_step(qw_sim *s, int64_t n) {
     const bool allow_fast = sched != QW_SCHED_GENERIC;
     for (int64_t i = 0; i < remaining; ++i) {
         const Box box = step_box(s);
-        int rc = launch_step(s, s->buf[s->cur], s->buf[1 - s->cur], box, allow_fast);
+        int rc = launch_step(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), box, allow_fast);
         if (rc) return rc;
         s->cur ^= 1; s->t += 1; s->radius += 1;
     }
@@ -400,7 +416,7 @@ int qw_step_inverse(qw_sim *s, int64_t n) {
     if (!s->has_coin) return fail(QW_ESTATE, "qw_step_inverse before qw_set_coin");
     if (!s->has_state) return fail(QW_ESTATE, "qw_step_inverse before qw_set_state");
     for (int64_t i = 0; i < n; ++i) {
-        int rc = launch_step_inverse(s, s->buf[s->cur], s->buf[1 - s->cur]);
+        int rc = launch_step_inverse(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur));
         if (rc) return rc;
         s->cur ^= 1; s->t -= 1; s->radius += 1;
     }
@@ -414,10 +430,10 @@ int qw_probabilities(const qw_sim *cs, void *out) {
     if (!out) return fail(QW_EINVAL, "out is NULL");
     if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
     const size_t bytes = (size_t)s->g.batch * (size_t)s->g.sites * (s->esize / 2);
-    if (is_device_ptr(out)) return launch_probabilities(s, s->buf[s->cur], out);
+    if (is_device_ptr(out)) return launch_probabilities(s, state_ptr(s, s->cur), out);
     int rc = ensure_scratch(s, bytes);
     if (rc) return rc;
-    rc = launch_probabilities(s, s->buf[s->cur], s->scratch);
+    rc = launch_probabilities(s, state_ptr(s, s->cur), s->scratch);
     if (rc) return rc;
     QW_CUDA(cudaMemcpyAsync(out, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
     QW_CUDA(cudaStreamSynchronize(s->stream));
@@ -431,10 +447,10 @@ int qw_moments(const qw_sim *cs, double *out) {
     if (!out) return fail(QW_EINVAL, "out is NULL");
     if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
     const size_t bytes = (size_t)s->g.batch * (s->g.dim == 1 ? 3 : 6) * sizeof(double);
-    if (is_device_ptr(out)) return launch_moments(s, s->buf[s->cur], out);
+    if (is_device_ptr(out)) return launch_moments(s, state_ptr(s, s->cur), out);
     int rc = ensure_scratch(s, bytes);
     if (rc) return rc;
-    rc = launch_moments(s, s->buf[s->cur], static_cast<double *>(s->scratch));
+    rc = launch_moments(s, state_ptr(s, s->cur), static_cast<double *>(s->scratch));
     if (rc) return rc;
     QW_CUDA(cudaMemcpyAsync(out, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
     QW_CUDA(cudaStreamSynchronize(s->stream));

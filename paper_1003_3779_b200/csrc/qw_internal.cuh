@@ -22,9 +22,13 @@ struct Geom {
     long long batch;
     long long em, en;        // 1D: em = 1, en = extent
     long long sites;         // em * en
-    long long pitch;         // complex elements per lattice row (>= en, padded)
-    long long walk_stride;   // em * pitch
+    long long pitch;         // complex elements per allocated row (>= en + 2*ghost, padded)
+    long long walk_stride;   // (em + 2*ghost) * pitch
     long long plane_stride;  // batch * walk_stride
+    int ghost;               // 2D: ghost ring of this many cells around every walk (0 in 1D); the
+                             // temporally blocked 2D kernel reads its halos from it (periodic: refreshed
+                             // from the opposite edge before every blocked launch; open: don't-care)
+    long long origin;        // element offset of site (0,0) of walk 0 inside a plane: ghost*pitch + ghost
 };
 
 enum CoinKind {
@@ -79,6 +83,10 @@ struct qw_sim {
     int last_sched, last_k;
     long long launches;
 
+    // TMA descriptors of the two state buffers (qw_step_blocked2d.cu), built lazily
+    alignas(64) unsigned char tmap[2][128];
+    bool tmap_ready;
+
     // scratch
     void *scratch;           // staging for host <-> device transposes and outputs
     size_t scratch_bytes;
@@ -87,6 +95,11 @@ struct qw_sim {
 };
 
 namespace qw {
+
+// pointer to site (0,0) of walk 0, plane 0 of state buffer i
+inline void *state_ptr(const qw_sim *s, int i) {
+    return static_cast<char *>(s->buf[i]) + (size_t)s->g.origin * s->esize;
+}
 
 // error reporting (qw_api.cu)
 int fail(int code, const char *fmt, ...);
@@ -127,6 +140,12 @@ int launch_step_blocked1d(qw_sim *s, const void *in, void *out, int k);
 // qw_step_resident1d.cu : one CTA per walk, all n steps on the SM (1D walks of <= 4096 sites)
 bool resident1d_eligible(const qw_sim *s);
 int launch_step_resident1d(qw_sim *s, const void *in, void *out, long long n);
+
+// qw_step_blocked2d.cu : k steps per launch, shared-memory tiles loaded by TMA (uniform coin, 2D natural)
+constexpr int QW_GHOST_2D = 16;
+bool blocked2d_eligible(const qw_sim *s);
+int blocked2d_max_k(const qw_sim *s);
+int launch_step_blocked2d(qw_sim *s, int in_buf, int out_buf, int k);
 
 // qw_reduce.cu
 int launch_probabilities(qw_sim *s, const void *state, void *out_dev);

@@ -74,10 +74,10 @@ int launch_delta(qw_sim *s, const long long *site, const double *cv) {
     double4 b = g.cdim == 4 ? make_double4(cv[4], cv[5], cv[6], cv[7]) : make_double4(0, 0, 0, 0);
     const unsigned blocks = (unsigned)((g.batch + 127) / 128);
     if (s->dtype == QW_C128)
-        delta_kernel<double><<<blocks, 128, 0, s->stream>>>(static_cast<double2 *>(s->buf[s->cur]), g.batch,
+        delta_kernel<double><<<blocks, 128, 0, s->stream>>>(static_cast<double2 *>(state_ptr(s, s->cur)), g.batch,
                                                              g.cdim, g.walk_stride, g.plane_stride, off, a, b);
     else
-        delta_kernel<float><<<blocks, 128, 0, s->stream>>>(static_cast<float2 *>(s->buf[s->cur]), g.batch,
+        delta_kernel<float><<<blocks, 128, 0, s->stream>>>(static_cast<float2 *>(state_ptr(s, s->cur)), g.batch,
                                                             g.cdim, g.walk_stride, g.plane_stride, off, a, b);
     QW_LAUNCH_CHECK(s, "delta_kernel");
     return QW_OK;

@@ -15,9 +15,10 @@
 
 namespace qw {
 
-constexpr int RES_M = 8;             // sites per thread
-constexpr int RES_MAX_THREADS = 512; // -> walks of up to 4096 sites
-constexpr int RES_SMALL_THREADS = 320;
+// Launch shapes (sites per thread M, threads, CTAs per SM).  256-thread CTAs put exactly two warps on
+// every SM sub-partition and two CTAs on every SM (the second CTA hides the first one's barrier);
+// M = 9 lets 256 threads hold the 2049-site walks of BASELINE.json:configs[4].
+constexpr int RES_MAX_SITES = 4096;
 
 template <typename R>
 struct Resident1dArgs {
@@ -131,8 +132,8 @@ struct ResidentUnroll {
     }
 };
 
-template <typename R, int M, int KIND, bool PHASES, bool OPEN, int MAXT>
-__global__ void __launch_bounds__(MAXT)
+template <typename R, int M, int KIND, bool PHASES, bool OPEN, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB)
 step_resident1d_kernel(const Resident1dArgs<R> a) {
     typedef typename Cx<R>::T V;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -204,12 +205,12 @@ step_resident1d_kernel(const Resident1dArgs<R> a) {
 
 bool resident1d_eligible(const qw_sim *s) {
     const Geom &g = s->g;
-    return g.dim == 1 && g.en <= (long long)RES_MAX_THREADS * RES_M && s->coin_mode != QW_COIN_PER_SITE &&
-           !s->d_broken && g.batch <= 0x7fffffffLL;
+    return g.dim == 1 && g.en <= RES_MAX_SITES && s->coin_mode != QW_COIN_PER_SITE && !s->d_broken &&
+           g.batch <= 0x7fffffffLL;
 }
 
-template <typename R, int KIND, bool PHASES>
-static int launch_resident_t(qw_sim *s, const void *in, void *out, long long n) {
+template <typename R, int M, int KIND, bool PHASES, int MAXT, int MINB>
+static int launch_resident_shape(qw_sim *s, const void *in, void *out, long long n) {
     typedef typename Cx<R>::T V;
     const Geom &g = s->g;
     Resident1dArgs<R> a;
@@ -222,27 +223,29 @@ static int launch_resident_t(qw_sim *s, const void *in, void *out, long long n) 
                          (g.boundary == QW_OPEN || (s->centre[0] - (s->radius + n + 1) >= 0 && s->centre[0] + (s->radius + n + 1) < g.en));
     a.window = cone_ok ? 1 : 0; a.centre = s->centre[0]; a.radius0 = s->radius;
     for (int i = 0; i < 8; ++i) a.coin[i] = (R)s->h_coin[i];
-    int threads = (int)((g.en + RES_M - 1) / RES_M);
+    int threads = (int)((g.en + M - 1) / M);
     threads = (threads + 31) / 32 * 32;
     const int nw = threads / 32;
-    const size_t smem = sizeof(V) * (size_t)(4 * nw + 4 + (PHASES ? (size_t)threads * (RES_M + 1) : 0));
+    const size_t smem = sizeof(V) * (size_t)(4 * nw + 4 + (PHASES ? (size_t)threads * (M + 1) : 0));
     auto launch = [&](auto kernel) -> int {
         if (smem > 48 * 1024)
             QW_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         kernel<<<(unsigned)g.batch, threads, smem, s->stream>>>(a);
         return QW_OK;
     };
-    // two register budgets: walks of <= 320*M sites may use up to 204 registers per thread
-    int rc;
-    if (threads <= RES_SMALL_THREADS)
-        rc = g.boundary == QW_OPEN ? launch(step_resident1d_kernel<R, RES_M, KIND, PHASES, true, RES_SMALL_THREADS>)
-                                   : launch(step_resident1d_kernel<R, RES_M, KIND, PHASES, false, RES_SMALL_THREADS>);
-    else
-        rc = g.boundary == QW_OPEN ? launch(step_resident1d_kernel<R, RES_M, KIND, PHASES, true, RES_MAX_THREADS>)
-                                   : launch(step_resident1d_kernel<R, RES_M, KIND, PHASES, false, RES_MAX_THREADS>);
+    int rc = g.boundary == QW_OPEN ? launch(step_resident1d_kernel<R, M, KIND, PHASES, true, MAXT, MINB>)
+                                   : launch(step_resident1d_kernel<R, M, KIND, PHASES, false, MAXT, MINB>);
     if (rc) return rc;
     QW_LAUNCH_CHECK(s, "step_resident1d_kernel");
     return QW_OK;
+}
+
+template <typename R, int KIND, bool PHASES>
+static int launch_resident_t(qw_sim *s, const void *in, void *out, long long n) {
+    const long long N = s->g.en;
+    if (N <= 256 * 8) return launch_resident_shape<R, 8, KIND, PHASES, 256, 2>(s, in, out, n);
+    if (N <= 256 * 9) return launch_resident_shape<R, 9, KIND, PHASES, 256, 2>(s, in, out, n);
+    return launch_resident_shape<R, 8, KIND, PHASES, 512, 1>(s, in, out, n);
 }
 
 int launch_step_resident1d(qw_sim *s, const void *in, void *out, long long n) {

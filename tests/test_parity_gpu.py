@@ -282,8 +282,35 @@ def test_resident_delta_start_with_light_cone(qw, oracle, dev, window):
     assert np.array_equal(got, gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)[0])
 
 
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.PERIODIC, qi.OPEN])
+@pytest.mark.parametrize("coin", ["grover", "hxh", "dft", "random"])
+def test_blocked_2d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, dtype, boundary, coin):
+    """P13 in 2D: TMA-staged shared-memory tiles advanced k steps in place == k fused single steps."""
+    rng = np.random.default_rng(12)
+    for extents, steps, k, batch in (((97, 130), 20, 0, 1), ((64, 64), 9, 3, 2), ((33, 200), 17, 1, 1), ((150, 41), 24, 7, 1)):
+        c = {"grover": qi.grover4, "hxh": qi.hadamard_x_hadamard, "dft": qi.dft4}[coin](dtype) if coin != "random" \
+            else qi.random_unitary(rng, 4).astype(dtype)
+        sites = extents[0] * extents[1]
+        w = qi.Workload("blk2d", 2, extents, batch, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
+                        state=qi.random_state(29, batch, sites, 4, dtype, normalise_per_walk=True))
+        a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_BLOCKED, k=k)
+        assert b[3]["sched"] == qw.QW_SCHED_BLOCKED
+        assert np.array_equal(a[0], b[0]), (extents, steps, k)
+    check_parity(w, b, oracle_run(oracle, w))
+
+
+def test_blocked_2d_delta_start_reaches_the_walls(qw, dev):
+    w = qi.k2(half=40, steps=100)
+    a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
+    b = gpu_run(qw, w, schedule=qw.QW_SCHED_BLOCKED, k=4, window=False)
+    assert np.array_equal(a[0], b[0])
+
+
 def test_blocked_schedule_rejected_where_it_does_not_apply(qw, dev):
     w = qi.k3(extents=(64, 64), steps=4, coin="dft")
+    w.lattice = qi.DIAGONAL
     h = qw.create_for(w)
     try:
         qw.load_state(h, w)
