@@ -339,7 +339,7 @@ def run_gpu(args):
 
     h = qw.create_for(w)
     if args.schedule is not None:
-        qw.qw_set_schedule(h, {"auto": 0, "generic": 1, "fused": 2, "blocked": 3, "resident": 4}[args.schedule], args.k)
+        qw.qw_set_schedule(h, {"auto": 0, "generic": 1, "fused": 2, "blocked": 3, "resident": 4, "tiled": 5}[args.schedule], args.k)
     if args.no_window:
         qw.qw_set_window(h, 0)
     stream = torch.cuda.current_stream()
@@ -459,9 +459,10 @@ def run_gpu(args):
     peak, peak_src = measured_peak()
     kernel_ms = step_ms / args.steps            # device time of the hot path per bench step, gaps included
     eff_gbs = site_updates_per_step * alg_bytes_per_site / (kernel_ms * 1e-3) / 1e9
-    sched_name = {0: "auto", 1: "generic", 2: "fused", 3: "blocked", 4: "resident"}.get(sched, str(sched))
+    sched_name = {0: "auto", 1: "generic", 2: "fused", 3: "blocked", 4: "resident", 5: "tiled"}.get(sched, str(sched))
     kname = {1: "step_scatter_kernel (generic)", 2: "step_scatter_kernel (fused coin+shift)",
-             3: "step_blocked1d_kernel", 4: "step_resident1d_kernel"}.get(sched, "?")
+             3: "step_blocked1d_kernel" if w.dim == 1 else "step_blocked2d_kernel", 4: "step_resident1d_kernel",
+             5: "step_tiled2d_kernel"}.get(sched, "?")
     if sched in (1, 2):
         roofline = {
             "bound": "hbm", "kernel": kname, "achieved": eff_gbs, "peak": peak, "unit": "GB/s", "frac": eff_gbs / peak,
@@ -523,7 +524,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="k1", choices=["k0", "k1", "k1c64", "k2", "k3hxh", "k3dft", "k4"])
     ap.add_argument("--walk-steps", type=int, default=None, help="walk steps per bench step (default: the config's)")
-    ap.add_argument("--schedule", default=None, choices=["auto", "generic", "fused", "blocked", "resident"])
+    ap.add_argument("--schedule", default=None, choices=["auto", "generic", "fused", "blocked", "resident", "tiled"])
     ap.add_argument("--k", type=int, default=0)
     ap.add_argument("--no-window", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

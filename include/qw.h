@@ -62,11 +62,15 @@ enum { QW_COIN_UNIFORM = 0, QW_COIN_PER_WALK = 1, QW_COIN_PER_SITE = 2 };
 
 /* Step schedules (qw_set_schedule).  All schedules compute bit-identical states. */
 enum {
-    QW_SCHED_AUTO = 0,     /* library picks: resident if a walk fits one CTA, else blocked / fused      */
+    QW_SCHED_AUTO = 0,     /* library picks: resident if a walk fits one CTA, else blocked (1D) / tiled
+                              (2D) / fused                                                              */
     QW_SCHED_GENERIC = 1,  /* one launch per step, one thread per site, every feature (reference kernel) */
     QW_SCHED_FUSED = 2,    /* one launch per step, vectorised fused coin+shift (HBM-bound)              */
-    QW_SCHED_BLOCKED = 3,  /* temporally blocked: k steps per HBM round trip                            */
-    QW_SCHED_RESIDENT = 4  /* one CTA per walk, state on the SM for all n steps                         */
+    QW_SCHED_BLOCKED = 3,  /* temporally blocked: k steps per HBM round trip (1D: register tiles per warp;
+                              2D: shared-memory tiles loaded by TMA)                                    */
+    QW_SCHED_RESIDENT = 4, /* one CTA per walk, state on the SM for all n steps                         */
+    QW_SCHED_TILED = 5     /* 2D temporally blocked, tiles held in REGISTERS by persistent CTAs with TMA
+                              prefetch; k in {2, 4, 6, 8}; honours the light-cone window                */
 };
 
 /* qw_get_info keys */
@@ -138,7 +142,8 @@ int qw_probabilities(const qw_sim *s, void *out);
  * mean and (population) variance are divided by the computed norm (eq. 4 fixes norm = 1). */
 int qw_moments(const qw_sim *s, double *out);
 
-/* Force a schedule (QW_SCHED_*); k = temporal block depth for QW_SCHED_BLOCKED (0 = library default).
+/* Force a schedule (QW_SCHED_*); k = temporal block depth for QW_SCHED_BLOCKED / QW_SCHED_TILED
+ * (0 = library default; QW_SCHED_TILED accepts 2, 4, 6 or 8, else QW_EINVAL).
  * QW_EUNSUPPORTED if the handle's configuration has no such kernel. */
 int qw_set_schedule(qw_sim *s, int schedule, int k);
 

@@ -20,7 +20,7 @@ QW_C64, QW_C128 = 0, 1
 QW_PERIODIC, QW_OPEN = 0, 1
 QW_NATURAL, QW_DIAGONAL = 0, 1
 QW_COIN_UNIFORM, QW_COIN_PER_WALK, QW_COIN_PER_SITE = 0, 1, 2
-QW_SCHED_AUTO, QW_SCHED_GENERIC, QW_SCHED_FUSED, QW_SCHED_BLOCKED, QW_SCHED_RESIDENT = 0, 1, 2, 3, 4
+QW_SCHED_AUTO, QW_SCHED_GENERIC, QW_SCHED_FUSED, QW_SCHED_BLOCKED, QW_SCHED_RESIDENT, QW_SCHED_TILED = 0, 1, 2, 3, 4, 5
 QW_INFO_LAUNCHES, QW_INFO_TIME, QW_INFO_LAST_SCHEDULE, QW_INFO_LAST_K, QW_INFO_STATE_BYTES, QW_INFO_WINDOW = range(6)
 
 # every symbol include/qw.h declares (tests/test_abi.py checks the header against this list)

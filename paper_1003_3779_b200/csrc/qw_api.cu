@@ -80,11 +80,12 @@ static int classify_coin(const double *C, int cdim, int dtype) {
 }
 
 // Source box of the next step (left = max(mid - extra - it, 1), ...).
-static Box step_box(const qw_sim *s) {
+// k = 1: the source sites of the next step; k > 1: the sites that can be non-zero after k more steps.
+static Box step_box(const qw_sim *s, long long k = 1) {
     const Geom &g = s->g;
     Box b{0, g.em - 1, 0, g.en - 1};
     if (!s->window_enabled || !s->window_valid) return b;
-    const long long r = s->radius + 1;   // pad of one site, like the paper's `extra`
+    const long long r = s->radius + k;   // k = 1: pad of one site, like the paper's `extra`
     auto clampdim = [&](long long c, long long ext, long long &lo, long long &hi) {
         long long l = c - r, h = c + r;
         if (g.boundary == QW_PERIODIC) { if (l < 0 || h >= ext) { l = 0; h = ext - 1; } }
@@ -357,7 +358,7 @@ int qw_step(qw_sim *s, int64_t n) {
     if (sched == QW_SCHED_AUTO)
         sched = resident1d_eligible(s) ? QW_SCHED_RESIDENT
               : (blocked1d_eligible(s) && n >= blocked1d_granule(s)) ? QW_SCHED_BLOCKED
-              : (blocked2d_eligible(s) && n >= 2 && !(s->window_enabled && s->window_valid)) ? QW_SCHED_BLOCKED : QW_SCHED_FUSED;
+              : (tiled2d_eligible(s) && n >= 2) ? QW_SCHED_TILED : QW_SCHED_FUSED;
     if (sched == QW_SCHED_RESIDENT) {
         if (!resident1d_eligible(s))
             return fail(QW_EUNSUPPORTED, "the resident schedule needs 1D walks of at most 4096 sites, no per-site matrices, no link mask");
@@ -371,8 +372,25 @@ int qw_step(qw_sim *s, int64_t n) {
         return fail(QW_EUNSUPPORTED, "the temporally blocked schedule needs a uniform coin without phases or link mask on a 1D "
                                      "lattice of >= %d sites or a natural 2D lattice of >= 32 x 32 sites",
                     32 * blocked1d_granule(s));
+    if (sched == QW_SCHED_TILED && !tiled2d_eligible(s))
+        return fail(QW_EUNSUPPORTED, "the tiled schedule needs a uniform coin without phases or link mask on a natural 2D "
+                                     "lattice of >= 32 x 32 sites");
+    if (sched == QW_SCHED_TILED && s->sched_k != 0 && s->sched_k != 2 && s->sched_k != 4 && s->sched_k != 6 && s->sched_k != 8)
+        return fail(QW_EINVAL, "the tiled schedule takes k = 2, 4, 6 or 8 (got %d)", s->sched_k);
     int64_t remaining = n;
     s->last_sched = sched; s->last_k = 1;
+    if (sched == QW_SCHED_TILED) {
+        // k-step launches, then the even part of the remainder; an odd last step goes through the fused kernel below
+        const int kmax = s->sched_k > 0 ? s->sched_k : 8;     // measured optimum on B200 (profiles/)
+        s->last_k = kmax;
+        while (remaining >= 2) {
+            const int kk = (int)(remaining >= kmax ? kmax : remaining / 2 * 2);
+            const Box box = step_box(s, kk);
+            int rc = launch_step_tiled2d(s, s->cur, 1 - s->cur, kk, box);
+            if (rc) return rc;
+            s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;
+        }
+    }
     if (sched == QW_SCHED_BLOCKED && s->g.dim == 2) {
         int kmax = s->sched_k > 0 ? s->sched_k : (s->dtype == QW_C128 ? 4 : 6);   // measured optima (profiles/)
         if (kmax > blocked2d_max_k(s)) kmax = blocked2d_max_k(s);
@@ -460,7 +478,7 @@ int qw_moments(const qw_sim *cs, double *out) {
 int qw_set_schedule(qw_sim *s, int schedule, int k) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
-    if (schedule < QW_SCHED_AUTO || schedule > QW_SCHED_RESIDENT) return fail(QW_EINVAL, "unknown schedule %d", schedule);
+    if (schedule < QW_SCHED_AUTO || schedule > QW_SCHED_TILED) return fail(QW_EINVAL, "unknown schedule %d", schedule);
     if (k < 0) return fail(QW_EINVAL, "k must be >= 0");
     s->sched = schedule; s->sched_k = k;
     return QW_OK;

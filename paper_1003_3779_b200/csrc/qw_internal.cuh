@@ -86,6 +86,8 @@ struct qw_sim {
     // TMA descriptors of the two state buffers (qw_step_blocked2d.cu), built lazily
     alignas(64) unsigned char tmap[2][128];
     bool tmap_ready;
+    alignas(64) unsigned char tmap_t[2][128];   // ... of the register-tiled kernel (qw_step_tiled2d.cuh)
+    bool tmap_t_ready;
 
     // scratch
     void *scratch;           // staging for host <-> device transposes and outputs
@@ -146,6 +148,14 @@ constexpr int QW_GHOST_2D = 16;
 bool blocked2d_eligible(const qw_sim *s);
 int blocked2d_max_k(const qw_sim *s);
 int launch_step_blocked2d(qw_sim *s, int in_buf, int out_buf, int k);
+int launch_ghost_refresh(qw_sim *s, int buf);     // periodic lattices: ghost ring := opposite edges
+
+// qw_step_tiled2d_*.cu : k in {2,4,6,8} steps per launch, persistent CTAs, tiles in REGISTERS, TMA prefetch
+// (uniform coin, 2D natural).  `box` = sites that can be non-zero after the launch (whole lattice if no window).
+bool tiled2d_eligible(const qw_sim *s);
+int launch_step_tiled2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
+int launch_tiled2d_f32(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
+int launch_tiled2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 
 // qw_reduce.cu
 int launch_probabilities(qw_sim *s, const void *state, void *out_dev);

@@ -271,22 +271,40 @@ static int launch_blocked2d_t(qw_sim *s, int in_buf, int out_buf, int k) {
     return QW_OK;
 }
 
+int launch_ghost_refresh(qw_sim *s, int buf) {
+    const Geom &g = s->g;
+    const long long per = 2LL * g.ghost * (g.en + 2 * g.ghost) + g.em * 2LL * g.ghost;
+    const long long nwp = 4 * g.batch;
+    dim3 grid((unsigned)((per + 255) / 256), (unsigned)(nwp < 64 ? nwp : 64));
+    if (s->dtype == QW_C128)
+        ghost_refresh_kernel<double2><<<grid, 256, 0, s->stream>>>(static_cast<double2 *>(s->buf[buf]), g.em, g.en, g.pitch,
+                                                                   g.walk_stride, g.ghost, nwp);
+    else
+        ghost_refresh_kernel<float2><<<grid, 256, 0, s->stream>>>(static_cast<float2 *>(s->buf[buf]), g.em, g.en, g.pitch,
+                                                                  g.walk_stride, g.ghost, nwp);
+    QW_LAUNCH_CHECK(s, "ghost_refresh_kernel");
+    return QW_OK;
+}
+
+bool tiled2d_eligible(const qw_sim *s) { return blocked2d_eligible(s); }
+
+// Register-tiled schedule: refresh the periodic halos, then dispatch on the dtype.
+int launch_step_tiled2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
+    if (s->g.boundary == QW_PERIODIC) {
+        int rc = launch_ghost_refresh(s, in_buf);
+        if (rc) return rc;
+    }
+    return s->dtype == QW_C128 ? launch_tiled2d_f64(s, in_buf, out_buf, k, box) : launch_tiled2d_f32(s, in_buf, out_buf, k, box);
+}
+
 int launch_step_blocked2d(qw_sim *s, int in_buf, int out_buf, int k) {
     const Geom &g = s->g;
     if (k < 1 || k > blocked2d_max_k(s)) return fail(QW_EINVAL, "blocked 2D step depth %d outside [1, %d]", k, blocked2d_max_k(s));
     int rc = build_tmaps(s);
     if (rc) return rc;
     if (g.boundary == QW_PERIODIC) {
-        const long long per = 2LL * g.ghost * (g.en + 2 * g.ghost) + g.em * 2LL * g.ghost;
-        const long long nwp = 4 * g.batch;
-        dim3 grid((unsigned)((per + 255) / 256), (unsigned)(nwp < 64 ? nwp : 64));
-        if (s->dtype == QW_C128)
-            ghost_refresh_kernel<double2><<<grid, 256, 0, s->stream>>>(static_cast<double2 *>(s->buf[in_buf]), g.em, g.en, g.pitch,
-                                                                       g.walk_stride, g.ghost, nwp);
-        else
-            ghost_refresh_kernel<float2><<<grid, 256, 0, s->stream>>>(static_cast<float2 *>(s->buf[in_buf]), g.em, g.en, g.pitch,
-                                                                      g.walk_stride, g.ghost, nwp);
-        QW_LAUNCH_CHECK(s, "ghost_refresh_kernel");
+        rc = launch_ghost_refresh(s, in_buf);
+        if (rc) return rc;
     }
 #define QW_B2D(R)                                                                             \
     switch (s->coin_kind) {                                                                   \

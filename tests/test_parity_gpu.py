@@ -308,6 +308,67 @@ def test_blocked_2d_delta_start_reaches_the_walls(qw, dev):
     assert np.array_equal(a[0], b[0])
 
 
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.PERIODIC, qi.OPEN])
+@pytest.mark.parametrize("coin", ["grover", "hxh", "dft", "random"])
+def test_tiled_2d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, dtype, boundary, coin):
+    """P13 in 2D, register tiles: persistent CTAs advancing TMA-prefetched tiles k steps in registers
+    (renamed shifts, shuffles along n, shared-memory slots along m) == k fused single steps.
+    Extents span several tiles with ragged tails, fewer tiles than SMs, more tiles than SMs, odd widths."""
+    rng = np.random.default_rng(13)
+    for extents, steps, k, batch in (((97, 130), 21, 0, 1), ((64, 64), 9, 2, 3), ((33, 200), 17, 4, 1),
+                                     ((150, 41), 26, 6, 1), ((500, 700), 16, 8, 1), ((35, 32), 8, 8, 2)):
+        c = {"grover": qi.grover4, "hxh": qi.hadamard_x_hadamard, "dft": qi.dft4}[coin](dtype) if coin != "random" \
+            else qi.random_unitary(rng, 4).astype(dtype)
+        sites = extents[0] * extents[1]
+        w = qi.Workload("til2d", 2, extents, batch, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
+                        state=qi.random_state(31, batch, sites, 4, dtype, normalise_per_walk=True))
+        a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k)
+        assert b[3]["sched"] == qw.QW_SCHED_TILED
+        assert np.array_equal(a[0], b[0]), (extents, steps, k)
+        if sites < 20000:
+            check_parity(w, b, oracle_run(oracle, w))
+
+
+@pytest.mark.parametrize("window", [True, False])
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+def test_tiled_2d_delta_start_reaches_the_walls(qw, dev, window, dtype):
+    """Light-cone window on the tiled schedule (only tiles meeting the cone are launched) and the
+    reflecting walls inside register tiles: the walker hits all four walls and comes back."""
+    w = qi.k2(half=40, steps=131)
+    w.dtype = np.dtype(dtype)
+    w.coin = w.coin.astype(dtype)
+    w.delta_coin = w.delta_coin.astype(dtype)
+    a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
+    for k in (0, 4):
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k, window=window)
+        assert b[3]["sched"] == qw.QW_SCHED_TILED
+        assert np.array_equal(a[0], b[0])
+        assert np.array_equal(a[1], b[1])
+    # off-centre start near a corner, walls met at different times
+    w.delta_site = (3, 70)
+    a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
+    b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, window=window)
+    assert np.array_equal(a[0], b[0])
+
+
+def test_tiled_2d_is_the_auto_schedule_and_rejects_bad_depths(qw, dev):
+    w = qi.k3(extents=(96, 80), steps=11, coin="dft")
+    a = gpu_run(qw, w)
+    assert a[3]["sched"] == qw.QW_SCHED_TILED and a[3]["k"] == 8
+    assert np.array_equal(a[0], gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)[0])
+    h = qw.create_for(w)
+    try:
+        qw.load_state(h, w)
+        qw.qw_set_schedule(h, qw.QW_SCHED_TILED, 3)
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_step(h, 4)
+        assert ei.value.code == qw.QW_EINVAL
+    finally:
+        qw.qw_destroy(h)
+
+
 def test_blocked_schedule_rejected_where_it_does_not_apply(qw, dev):
     w = qi.k3(extents=(64, 64), steps=4, coin="dft")
     w.lattice = qi.DIAGONAL
