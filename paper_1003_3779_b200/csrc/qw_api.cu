@@ -381,7 +381,7 @@ int qw_step(qw_sim *s, int64_t n) {
     s->last_sched = sched; s->last_k = 1;
     if (sched == QW_SCHED_TILED) {
         // k-step launches, then the even part of the remainder; an odd last step goes through the fused kernel below
-        const int kmax = s->sched_k > 0 ? s->sched_k : 8;     // measured optimum on B200 (profiles/)
+        const int kmax = s->sched_k > 0 ? s->sched_k : (s->dtype == QW_C128 ? 6 : 8);   // measured optima on B200 (profiles/)
         s->last_k = kmax;
         while (remaining >= 2) {
             const int kk = (int)(remaining >= kmax ? kmax : remaining / 2 * 2);

@@ -53,6 +53,13 @@ template <typename R> __device__ __forceinline__ cplx<R> cx_sub(cplx<R> a, cplx<
 template <typename R> __device__ __forceinline__ cplx<R> cx_scale(R s, cplx<R> a) {
     return cplx<R>{mul_rn(s, a.re), mul_rn(s, a.im)};
 }
+// s * a + b,  s * a - b  with a real scale s
+template <typename R> __device__ __forceinline__ cplx<R> cx_fma_r(R s, cplx<R> a, cplx<R> b) {
+    return cplx<R>{fma_rn(s, a.re, b.re), fma_rn(s, a.im, b.im)};
+}
+template <typename R> __device__ __forceinline__ cplx<R> cx_fms_r(R s, cplx<R> a, cplx<R> b) {
+    return cplx<R>{fma_rn(s, a.re, -b.re), fma_rn(s, a.im, -b.im)};
+}
 // i * a,  -i * a   (exact)
 template <typename R> __device__ __forceinline__ cplx<R> cx_muli(cplx<R> a)  { return cplx<R>{-a.im, a.re}; }
 template <typename R> __device__ __forceinline__ cplx<R> cx_mulni(cplx<R> a) { return cplx<R>{a.im, -a.re}; }
@@ -83,23 +90,27 @@ __device__ __forceinline__ void apply_coin(const R *__restrict__ C, cplx<R> (&v)
             v[a].im = fma_rn(dg, v[a].im, gs.im);
         }
     } else if constexpr (KIND == COIN_HXH4 && CD == 4) {
-        // h * (H (x) H) with c = 2j+k: butterfly over k, then over j, then one scale
+        // h * (H (x) H) with c = 2j+k.  The scale rides on the first butterfly (over k) as FMAs:
+        // h*(x + y) = fma(h, x, h*y), then the butterfly over j: 2 mul + 4 fma + 4 add per real component.
+        // For h = 1/2 (the unitary case) the scaling is exact, i.e. this equals h * ((x + y) + (z + w)) bit for bit.
         const R h = C[0];
-        cplx<R> a0 = cx_add(v[0], v[1]), a1 = cx_sub(v[0], v[1]);
-        cplx<R> a2 = cx_add(v[2], v[3]), a3 = cx_sub(v[2], v[3]);
-        v[0] = cx_scale(h, cx_add(a0, a2));
-        v[1] = cx_scale(h, cx_add(a1, a3));
-        v[2] = cx_scale(h, cx_sub(a0, a2));
-        v[3] = cx_scale(h, cx_sub(a1, a3));
+        const cplx<R> t1 = cx_scale(h, v[1]), t3 = cx_scale(h, v[3]);
+        const cplx<R> a0 = cx_fma_r(h, v[0], t1), a1 = cx_fms_r(h, v[0], t1);
+        const cplx<R> a2 = cx_fma_r(h, v[2], t3), a3 = cx_fms_r(h, v[2], t3);
+        v[0] = cx_add(a0, a2);
+        v[1] = cx_add(a1, a3);
+        v[2] = cx_sub(a0, a2);
+        v[3] = cx_sub(a1, a3);
     } else if constexpr (KIND == COIN_DFT4 && CD == 4) {
-        // h * i^(ab): radix-2 decimation: e = v0 +- v2, o = v1 +- v3
+        // h * i^(ab): radix-2 decimation e = h*(v0 +- v2), o = h*(v1 +- v3) with the scale folded into FMAs
         const R h = C[0];
-        cplx<R> e0 = cx_add(v[0], v[2]), e1 = cx_sub(v[0], v[2]);
-        cplx<R> o0 = cx_add(v[1], v[3]), o1 = cx_muli(cx_sub(v[1], v[3]));
-        v[0] = cx_scale(h, cx_add(e0, o0));
-        v[1] = cx_scale(h, cx_add(e1, o1));
-        v[2] = cx_scale(h, cx_sub(e0, o0));
-        v[3] = cx_scale(h, cx_sub(e1, o1));
+        const cplx<R> t2 = cx_scale(h, v[2]), t3 = cx_scale(h, v[3]);
+        const cplx<R> e0 = cx_fma_r(h, v[0], t2), e1 = cx_fms_r(h, v[0], t2);
+        const cplx<R> o0 = cx_fma_r(h, v[1], t3), o1 = cx_muli(cx_fms_r(h, v[1], t3));
+        v[0] = cx_add(e0, o0);
+        v[1] = cx_add(e1, o1);
+        v[2] = cx_sub(e0, o0);
+        v[3] = cx_sub(e1, o1);
     } else {
         cplx<R> out[CD];
 #pragma unroll

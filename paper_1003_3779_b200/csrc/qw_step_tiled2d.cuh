@@ -14,7 +14,8 @@
 //                                c3[i][(j+s) mod RN]  (moves n-1)   c2[(i+s) mod RM][j]  (moves m-1)
 //          so only what crosses a patch edge moves: per step RM elements of c0 / c3 go to the
 //          neighbouring lane through warp shuffles and RN elements of c1 / c2 go to the neighbouring
-//          warp through a double-buffered shared-memory slot and ONE __syncthreads.
+//          warp through a double-buffered shared-memory slot guarded by one mbarrier per warp: a
+//          warp waits for its two neighbours only, never for the whole CTA.
 //          The K steps are fully unrolled, so every register index is a compile-time constant.
 //   walls  (open lattice = broken outward links, PAPER.md:94-101 with RBL = 0): at a wall site the
 //          outgoing component overrides what would have come in from outside, with the opposite
@@ -34,8 +35,8 @@
 namespace qw {
 
 template <typename R> struct T2dCfg;
-template <> struct T2dCfg<float>  { static constexpr int RM = 8, RN = 2, W = 8; };   // 64 x 64 sites, 128 KiB stage
-template <> struct T2dCfg<double> { static constexpr int RM = 4, RN = 2, W = 8; };   // 32 x 64 sites, 128 KiB stage
+template <> struct T2dCfg<float>  { static constexpr int RM = 4, RN = 2, W = 16; static constexpr bool NSYNC = false; };  // 64 x 64 sites, 128 KiB stage
+template <> struct T2dCfg<double> { static constexpr int RM = 4, RN = 2, W = 8;  static constexpr bool NSYNC = true; };   // 32 x 64 sites, 128 KiB stage
 
 template <typename R>
 struct Tiled2dArgs {
@@ -58,6 +59,9 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     uint32_t done;
@@ -123,10 +127,12 @@ struct Walls {
 };
 
 // One walk step, S = number of steps already applied to this tile (compile time).
-// xb = exchange slots of this step's parity: V xb[W][2][RN][32].
+// xb = exchange slots of this step's parity: V xb[W][2][RN][32]; xbar = their W "slot of warp w is full"
+// mbarriers; bit (S & 1) of xph = the phase parity to wait for.  A warp only waits for its two neighbours:
+// they can never be more than one step apart, so the double-buffered slots and barriers are race-free.
 template <typename R, int RM, int RN, int W, int KIND, bool OPEN, int S>
-__device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename Cx<R>::T *xb, int lane, int wid,
-                                     bool wall_tile, const Walls &wl) {
+__device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename Cx<R>::T *xb, uint64_t *xbar, uint32_t &xph,
+                                     int lane, int wid, bool wall_tile, const Walls &wl) {
     typedef typename Cx<R>::T V;
     // ---- coin (eq. 1) on every site of the patch, in place
 #pragma unroll
@@ -154,6 +160,15 @@ __device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename C
         z2.x = p.c2[P2][j].re; z2.y = p.c2[P2][j].im;
         xb[((wid * 2 + 0) * RN + j) * 32 + lane] = z1;
         xb[((wid * 2 + 1) * RN + j) * 32 + lane] = z2;
+    }
+    // NSYNC: neighbour-only synchronisation through mbarriers; otherwise one __syncthreads per step
+    constexpr bool NSYNC = T2dCfg<R>::NSYNC;
+    uint32_t par = 0;
+    if constexpr (NSYNC) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(xbar + wid);
+        par = (xph >> (S & 1)) & 1u;
+        xph ^= 1u << (S & 1);
     }
     if (OPEN && wall_tile) {                       // CTA-uniform branch
         // reflecting walls (RBL = 0): the outgoing component stays with the opposite coin
@@ -189,12 +204,14 @@ __device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename C
                 if (wl.jl == j) p.c0[i][t2d_mod(j - S - 1, RN)] = f0;
             }
         }
-        __syncthreads();
+        if constexpr (!NSYNC) __syncthreads();
         if (wid > 0) {
+            if constexpr (NSYNC) mbar_wait(xbar + wid - 1, par);
 #pragma unroll
             for (int j = 0; j < RN; ++j) p.c1[Q1][j] = cx_load<R>(xb + (((wid - 1) * 2 + 0) * RN + j) * 32 + lane);
         }
         if (wid < W - 1) {
+            if constexpr (NSYNC) mbar_wait(xbar + wid + 1, par);
 #pragma unroll
             for (int j = 0; j < RN; ++j) p.c2[P2][j] = cx_load<R>(xb + (((wid + 1) * 2 + 1) * RN + j) * 32 + lane);
         }
@@ -215,12 +232,14 @@ __device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename C
             p.c0[i][Q0] = shfl_up1(p.c0[i][Q0]);
             p.c3[i][P3] = shfl_down1(p.c3[i][P3]);
         }
-        __syncthreads();
+        if constexpr (!NSYNC) __syncthreads();
         if (wid > 0) {
+            if constexpr (NSYNC) mbar_wait(xbar + wid - 1, par);
 #pragma unroll
             for (int j = 0; j < RN; ++j) p.c1[Q1][j] = cx_load<R>(xb + (((wid - 1) * 2 + 0) * RN + j) * 32 + lane);
         }
         if (wid < W - 1) {
+            if constexpr (NSYNC) mbar_wait(xbar + wid + 1, par);
 #pragma unroll
             for (int j = 0; j < RN; ++j) p.c2[P2][j] = cx_load<R>(xb + (((wid + 1) * 2 + 1) * RN + j) * 32 + lane);
         }
@@ -229,10 +248,10 @@ __device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename C
 
 template <typename R, int RM, int RN, int W, int KIND, bool OPEN, int S, int K>
 struct Steps {
-    static __device__ __forceinline__ void run(Patch<R, RM, RN> &p, const R *C, typename Cx<R>::T *xch, int lane, int wid,
-                                               bool wall_tile, const Walls &wl) {
-        step<R, RM, RN, W, KIND, OPEN, S>(p, C, xch + (S & 1) * (W * 2 * RN * 32), lane, wid, wall_tile, wl);
-        if constexpr (S + 1 < K) Steps<R, RM, RN, W, KIND, OPEN, S + 1, K>::run(p, C, xch, lane, wid, wall_tile, wl);
+    static __device__ __forceinline__ void run(Patch<R, RM, RN> &p, const R *C, typename Cx<R>::T *xch, uint64_t *xbar,
+                                               uint32_t &xph, int lane, int wid, bool wall_tile, const Walls &wl) {
+        step<R, RM, RN, W, KIND, OPEN, S>(p, C, xch + (S & 1) * (W * 2 * RN * 32), xbar + (S & 1) * W, xph, lane, wid, wall_tile, wl);
+        if constexpr (S + 1 < K) Steps<R, RM, RN, W, KIND, OPEN, S + 1, K>::run(p, C, xch, xbar, xph, lane, wid, wall_tile, wl);
     }
 };
 
@@ -242,7 +261,7 @@ template <typename R> constexpr size_t tiled2d_smem_bytes() {
     typedef T2dCfg<R> G;
     return (size_t)4 * (G::W * G::RM) * (32 * G::RN) * sizeof(typename Cx<R>::T)      // TMA stage
          + (size_t)2 * G::W * 2 * G::RN * 32 * sizeof(typename Cx<R>::T)              // exchange slots
-         + 16;                                                                        // mbarrier
+         + (size_t)(2 * G::W + 2) * 8;                                                // mbarriers
 }
 
 template <typename R, int KIND, bool OPEN, int K>
@@ -262,7 +281,8 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
     extern __shared__ __align__(128) unsigned char smem_raw[];
     V *stage = reinterpret_cast<V *>(smem_raw);                    // stage[c][row][col]
     V *xch = stage + 4 * PLANE;                                    // xch[parity][warp][2][RN][32]
-    uint64_t *bar = reinterpret_cast<uint64_t *>(xch + 2 * W * 2 * RN * 32);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(xch + 2 * W * 2 * RN * 32);   // "stage is full"
+    uint64_t *xbar = bar + 2;                                      // xbar[parity][warp]: "slot of the warp is full"
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const long long per_walk = (long long)a.tiles_m * a.tiles_n;
@@ -280,13 +300,14 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
 
     if (tid == 0) {
         t2d::mbar_init(bar, 1);
+        for (int i = 0; i < 2 * W; ++i) t2d::mbar_init(xbar + i, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     long long t = blockIdx.x;
     if (tid == 0 && t < a.total_tiles) issue(t);
     const R *C = a.coin;                                           // kernel parameter = constant bank operands
-    uint32_t phase = 0;
+    uint32_t phase = 0, xph = 0;
 
     for (; t < a.total_tiles; t += gridDim.x) {
         const long long w = t / per_walk;
@@ -321,7 +342,7 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
             wl.jl = (jl >= 0 && jl < RN) ? (int)jl : -1;
             wl.jr = (jr >= 0 && jr < RN) ? (int)jr : -1;
         }
-        t2d::Steps<R, RM, RN, W, KIND, OPEN, 0, K>::run(p, C, xch, lane, wid, wall_tile, wl);
+        t2d::Steps<R, RM, RN, W, KIND, OPEN, 0, K>::run(p, C, xch, xbar, xph, lane, wid, wall_tile, wl);
 
         // ---- store the valid interior straight from registers: psi_c(i, j) after K steps sits at
         //      c0[i][(j-K) mod RN], c1[(i-K) mod RM][j], c2[(i+K) mod RM][j], c3[i][(j+K) mod RN]
