@@ -88,11 +88,11 @@ def coin_cost(w):
         return instr, flops
     if w.coin_mode == qi.COIN_UNIFORM and np.all(c.imag == 0) and np.all(np.abs(c) == abs(c[0, 0])):
         if np.array_equal(np.sign(c.real), np.sign(qi.hadamard_x_hadamard().real)):
-            return 24, 24
+            return 20, 24          # 2 mul + 4 fma + 4 add per real component; 16 add + 8 mul algorithmic
     if w.coin_mode == qi.COIN_UNIFORM and np.array_equal(c, qi.grover4(c.dtype)):
         return 16, 24
     if w.coin_mode == qi.COIN_UNIFORM and np.array_equal(c, qi.dft4(c.dtype)):
-        return 24, 24
+        return 20, 24
     return 64, 120
 
 
