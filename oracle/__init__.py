@@ -10,7 +10,11 @@ from .oracle import (  # noqa: F401
     build,
     dense_unitary,
     moments,
+    philox4x32_10,
     probabilities,
+    rbl_mask,
     step,
     step_inverse,
+    step_inverse_rbl,
+    step_rbl,
 )

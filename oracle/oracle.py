@@ -44,8 +44,15 @@ def _load():
         lib.qwo_moments.argtypes = [ctypes.c_int, i64p, ctypes.c_int64, vp, vp]
         lib.qwo_dense_unitary.argtypes = [ctypes.c_int, i64p, ctypes.c_int, ctypes.c_int,
                                           ctypes.c_int, vp, vp, vp]
+        lib.qwo_step_rbl.argtypes = [ctypes.c_int, i64p, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp,
+                                     ctypes.c_double, ctypes.c_uint64, ctypes.c_int64, vp, ctypes.c_int64]
+        lib.qwo_step_inverse_rbl.argtypes = lib.qwo_step_rbl.argtypes
+        lib.qwo_rbl_mask.argtypes = [ctypes.c_int, i64p, ctypes.c_int64, ctypes.c_int, ctypes.c_int,
+                                     ctypes.c_double, ctypes.c_uint64, ctypes.c_int64, vp]
+        lib.qwo_philox4x32_10.argtypes = [vp, vp, vp]
+        lib.qwo_philox4x32_10.restype = None
         for f in (lib.qwo_step, lib.qwo_step_inverse, lib.qwo_probabilities, lib.qwo_moments,
-                  lib.qwo_dense_unitary):
+                  lib.qwo_dense_unitary, lib.qwo_step_rbl, lib.qwo_step_inverse_rbl, lib.qwo_rbl_mask):
             f.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -141,3 +148,48 @@ def dense_unitary(extents, coin, *, boundary=PERIODIC, coin_mode=COIN_UNIFORM, l
     if rc:
         raise ValueError("oracle rejected the arguments")
     return U
+
+
+def _run_rbl(fn, extents, coin, state, n, p, seed, t0, boundary, coin_mode, batch, lattice):
+    dim, ext, sites = _ext(extents)
+    cdim = 2 * dim
+    _state(state, batch, sites, cdim)
+    coin = _coin(coin, cdim, coin_mode, batch, sites)
+    rc = fn(dim, ext, batch, boundary, lattice, coin_mode, coin.ctypes.data, float(p), int(seed), int(t0),
+            state.ctypes.data, int(n))
+    if rc:
+        raise ValueError("oracle rejected the arguments (rc=%d)" % rc)
+    return state
+
+
+def step_rbl(extents, coin, state, n, p, seed, *, t0=0, boundary=PERIODIC, coin_mode=COIN_UNIFORM, batch=1,
+             lattice=NATURAL):
+    """Apply U(t0) .. U(t0+n-1) in place, every link redrawn broken with probability p at every step
+    (eqs. 9-10; Philox4x32-10 keyed by ``seed``, see qw_oracle.cpp)."""
+    return _run_rbl(_load().qwo_step_rbl, extents, coin, state, n, p, seed, t0, boundary, coin_mode, batch, lattice)
+
+
+def step_inverse_rbl(extents, coin, state, n, p, seed, *, t0, boundary=PERIODIC, coin_mode=COIN_UNIFORM, batch=1,
+                     lattice=NATURAL):
+    """Undo steps t0-1 .. t0-n of a random-broken-links walk in place (t0 = current time)."""
+    return _run_rbl(_load().qwo_step_inverse_rbl, extents, coin, state, n, p, seed, t0, boundary, coin_mode, batch,
+                    lattice)
+
+
+def rbl_mask(extents, p, seed, t, *, boundary=PERIODIC, batch=1, lattice=NATURAL):
+    """The broken-link mask [batch][site][coin] (uint8) of step t, in the form ``step(..., broken=)`` takes."""
+    dim, ext, sites = _ext(extents)
+    out = np.empty((batch, sites, 2 * dim), dtype=np.uint8)
+    rc = _load().qwo_rbl_mask(dim, ext, batch, boundary, lattice, float(p), int(seed), int(t), out.ctypes.data)
+    if rc:
+        raise ValueError("oracle rejected the arguments")
+    return out
+
+
+def philox4x32_10(counter, key):
+    """The raw generator: 4 counter words, 2 key words -> 4 output words (uint32)."""
+    c = np.ascontiguousarray(counter, dtype=np.uint32)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.empty(4, dtype=np.uint32)
+    _load().qwo_philox4x32_10(c.ctypes.data, k.ctypes.data, out.ctypes.data)
+    return out

@@ -28,6 +28,19 @@
 //            then treated exactly like the open-boundary case.  The caller supplies a
 //            symmetric mask (both ends of a link agree); the oracle does not check that.
 //
+//   random broken links ("random broken links (termed RBL) technique", ref. [12]; eqs. 9-10):
+//            qwo_step_rbl redraws the link states at EVERY step: each link of the lattice is broken
+//            independently with probability p.  The paper names no generator; reading R27:
+//            the state of a link is a pure function of (seed, walk, step, link) through the counter-based
+//            generator Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11):
+//              link    = (owner site, axis): the owner is the end from which the link points in the
+//                        positive direction (dm > 0, or dm = 0 and dn > 0); axis = 0 for links along n
+//                        (natural / 1D) or along (+1,+1) (diagonal), 1 for links along m or (+1,-1)
+//              counter = (owner index low 32 bits, owner index high bits, step t, walk w), key = seed
+//              broken  iff output word [axis] < floor(p * 2^32)
+//            Links that leave an open lattice stay broken regardless.  Both ends of a link evaluate the
+//            same function, so U(t) is unitary (pinned by the dense form).
+//
 // Parity status: every function here is pinned by tests/test_oracle_pins.py
 // (hand/brute-force path sums, spectral closed form via FFT, Kronecker-product dense
 // unitary, exact degenerate coins, invariants).  Nothing is "parity unpinned".
@@ -89,6 +102,47 @@ inline bool target(const Lattice& L, int64_t m, int64_t n, int a, int64_t* tm, i
     return true;
 }
 
+// Philox4x32-10, written from the published round function: two 32x32->64 multiplies by the constants
+// M0, M1, the high halves XORed with the other counter words and the key, key bumped by the Weyl
+// constants W0, W1 after every round; 10 rounds.
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    const uint64_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = M0 * c0, p1 = M1 * c2;
+        const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n1 = lo1, n2 = hi0 ^ c3 ^ k1, n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Random broken links: is the link that component a of site (m,n) of walk w points along broken at step t?
+// (header: "random broken links").  The link is assumed to stay inside the lattice (target() returned true
+// with (tm,tn)).
+inline bool rbl_broken(const Lattice& L, int64_t w, int64_t m, int64_t n, int a, int64_t tm, int64_t tn,
+                       int64_t t, uint64_t thr, uint64_t seed) {
+    const int dm = L.dir[a][0], dn = L.dir[a][1];
+    const bool positive = dm > 0 || (dm == 0 && dn > 0);
+    const int64_t owner = positive ? (m * L.en + n) : (tm * L.en + tn);
+    int axis;
+    if (dm != 0 && dn != 0) axis = (dm * dn > 0) ? 0 : 1;      // diagonal lattice
+    else axis = (dm != 0) ? 1 : 0;                             // natural lattice / 1D
+    const uint32_t ctr[4] = { (uint32_t)((uint64_t)owner & 0xffffffffu), (uint32_t)((uint64_t)owner >> 32),
+                              (uint32_t)((uint64_t)t & 0xffffffffu), (uint32_t)((uint64_t)w & 0xffffffffu) };
+    const uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
+    uint32_t out[4];
+    philox4x32_10(ctr, key, out);
+    return (uint64_t)out[axis] < thr;
+}
+
+inline uint64_t rbl_threshold(double p) {       // floor(p * 2^32), p in [0, 1]
+    return (uint64_t)(p * 4294967296.0);
+}
+
 inline const cplx* coin_at(const cplx* coin, int coin_mode, const Lattice& L, int64_t w, int64_t x) {
     const int64_t c2 = (int64_t)L.cdim * L.cdim;
     if (coin_mode == 0) return coin;
@@ -104,8 +158,10 @@ extern "C" {
 // coin: row-major cdim x cdim complex; coin_mode 0: one matrix, 1: batch matrices, 2: batch*sites.
 // broken: nullptr, or [batch][site][coin] bytes (non-zero = the link component `coin` of that
 //         site would cross is broken), constant over the n steps.
-int qwo_step(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
-             int coin_mode, const double* coin_, const uint8_t* broken, double* state_, int64_t n) {
+static int step_core(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
+                     int coin_mode, const double* coin_, const uint8_t* broken, bool rbl, double p, uint64_t seed,
+                     int64_t t0, double* state_, int64_t n) {
+    const uint64_t thr = rbl ? rbl_threshold(p) : 0;
     Lattice L;
     if (!make_lattice(dim, extents, boundary, lattice_kind, &L) || batch < 1 || n < 0) return -1;
     const cplx* coin = reinterpret_cast<const cplx*>(coin_);
@@ -134,6 +190,7 @@ int qwo_step(int dim, const int64_t* extents, int64_t batch, int boundary, int l
                         int64_t tm, tn;
                         bool ok = target(L, m, nn, a, &tm, &tn);
                         if (ok && broken && broken[(w * L.sites + x) * cd + a]) ok = false;
+                        if (ok && rbl && rbl_broken(L, w, m, nn, a, tm, tn, t0 + step, thr, seed)) ok = false;
                         if (ok) next[(tm * L.en + tn) * cd + a] = phi[x * cd + a];
                         else    next[x * cd + (cd - 1 - a)] = phi[x * cd + a];
                     }
@@ -145,9 +202,46 @@ int qwo_step(int dim, const int64_t* extents, int64_t batch, int boundary, int l
     return 0;
 }
 
+int qwo_step(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
+             int coin_mode, const double* coin_, const uint8_t* broken, double* state_, int64_t n) {
+    return step_core(dim, extents, batch, boundary, lattice_kind, coin_mode, coin_, broken, false, 0.0, 0, 0, state_, n);
+}
+
+// n applications of U(t), t = t0 .. t0+n-1, with the links redrawn at every step (header: "random broken links";
+// PAPER.md:84, eqs. 9-10).  p in [0, 1].
+int qwo_step_rbl(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
+                 int coin_mode, const double* coin_, double p, uint64_t seed, int64_t t0, double* state_, int64_t n) {
+    if (!(p >= 0.0 && p <= 1.0) || t0 < 0) return -1;
+    return step_core(dim, extents, batch, boundary, lattice_kind, coin_mode, coin_, nullptr, true, p, seed, t0, state_, n);
+}
+
+// The link mask of step t as qwo_step's `broken` argument would take it: mask[w][x][a] = 1 iff the link component a
+// of site x points along is broken at step t (links leaving an open lattice are not marked: they are always broken).
+int qwo_rbl_mask(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
+                 double p, uint64_t seed, int64_t t, uint8_t* mask) {
+    Lattice L;
+    if (!make_lattice(dim, extents, boundary, lattice_kind, &L) || batch < 1 || !(p >= 0.0 && p <= 1.0)) return -1;
+    const uint64_t thr = rbl_threshold(p);
+    for (int64_t w = 0; w < batch; ++w)
+        for (int64_t m = 0; m < L.em; ++m)
+            for (int64_t nn = 0; nn < L.en; ++nn)
+                for (int a = 0; a < L.cdim; ++a) {
+                    int64_t tm, tn;
+                    const bool ok = target(L, m, nn, a, &tm, &tn);
+                    mask[(w * L.sites + m * L.en + nn) * L.cdim + a] =
+                        (ok && rbl_broken(L, w, m, nn, a, tm, tn, t, thr, seed)) ? 1 : 0;
+                }
+    return 0;
+}
+
+// The generator alone (known-answer pin).
+void qwo_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) { philox4x32_10(ctr, key, out); }
+
 // n applications of U^dagger = (I (x) C^dagger) S^dagger (reversibility pin).
-int qwo_step_inverse(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
-                     int coin_mode, const double* coin_, const uint8_t* broken, double* state_, int64_t n) {
+static int inverse_core(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
+                        int coin_mode, const double* coin_, const uint8_t* broken, bool rbl, double p, uint64_t seed,
+                        int64_t t0, double* state_, int64_t n) {
+    const uint64_t thr = rbl ? rbl_threshold(p) : 0;
     Lattice L;
     if (!make_lattice(dim, extents, boundary, lattice_kind, &L) || batch < 1 || n < 0) return -1;
     const cplx* coin = reinterpret_cast<const cplx*>(coin_);
@@ -165,6 +259,8 @@ int qwo_step_inverse(int dim, const int64_t* extents, int64_t batch, int boundar
                         int64_t tm, tn;
                         bool ok = target(L, m, nn, a, &tm, &tn);
                         if (ok && broken && broken[(w * L.sites + x) * cd + a]) ok = false;
+                        // inverse step number `step` undoes the forward step t0 - 1 - step
+                        if (ok && rbl && rbl_broken(L, w, m, nn, a, tm, tn, t0 - 1 - step, thr, seed)) ok = false;
                         phi[x * cd + a] = ok ? psi[(tm * L.en + tn) * cd + a] : psi[x * cd + (cd - 1 - a)];
                     }
                 }
@@ -180,6 +276,18 @@ int qwo_step_inverse(int dim, const int64_t* extents, int64_t batch, int boundar
         }
     }
     return 0;
+}
+
+int qwo_step_inverse(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
+                     int coin_mode, const double* coin_, const uint8_t* broken, double* state_, int64_t n) {
+    return inverse_core(dim, extents, batch, boundary, lattice_kind, coin_mode, coin_, broken, false, 0.0, 0, 0, state_, n);
+}
+
+// Undo the n steps t0-1, t0-2, ..., t0-n of a random-broken-links walk (t0 = current time).
+int qwo_step_inverse_rbl(int dim, const int64_t* extents, int64_t batch, int boundary, int lattice_kind,
+                         int coin_mode, const double* coin_, double p, uint64_t seed, int64_t t0, double* state_, int64_t n) {
+    if (!(p >= 0.0 && p <= 1.0) || t0 < n) return -1;
+    return inverse_core(dim, extents, batch, boundary, lattice_kind, coin_mode, coin_, nullptr, true, p, seed, t0, state_, n);
 }
 
 // P[w][x] = sum_a |psi[w][x][a]|^2     (Figs. 3-4)
