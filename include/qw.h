@@ -116,6 +116,21 @@ int qw_set_site_phases(qw_sim *s, const void *phases);
  * same bit (not checked).  NULL removes the mask. */
 int qw_set_broken_links(qw_sim *s, const uint8_t *mask);
 
+/* Random broken links redrawn at EVERY step ("random broken links (termed RBL) technique";
+ * PAPER.md:92-102 eqs. 9-10): with enable != 0, step t (t = steps applied since the last qw_set_state*)
+ * applies U(t) in which every link of the lattice is broken independently with probability p in [0, 1];
+ * a broken link acts as in qw_set_broken_links.  The paper names no generator; the state of a link is
+ * the pure function (reading R27)
+ *     broken  <=>  Philox4x32-10(counter = (owner lo32, owner hi32, t lo32, walk lo32), key = seed)[axis]
+ *                  < floor(p * 2^32)
+ * owner = site index of the end from which the link points in the positive direction (dm > 0, or
+ * dm = 0 and dn > 0); axis = 0 for links along n (1D, natural) or along (+1,+1) (diagonal), 1 for links
+ * along m or along (+1,-1).  Both ends of a link see the same value, so every U(t) is unitary, and
+ * qw_step_inverse undoes the same sequence (QW_ESTATE if it would pass t = 0).  Links leaving a QW_OPEN
+ * lattice stay broken; a static mask, if set, is OR-ed in.  enable = 0 switches the redraw off.
+ * QW_EINVAL for p outside [0, 1]. */
+int qw_set_random_broken_links(qw_sim *s, int enable, double p, uint64_t seed);
+
 /* Set the state from AoS amplitudes [batch][site][coin]; resets the step counter.  The library
  * never normalises (eq. 4 is the caller's responsibility). */
 int qw_set_state(qw_sim *s, const void *amps);

@@ -26,7 +26,7 @@ QW_INFO_LAUNCHES, QW_INFO_TIME, QW_INFO_LAST_SCHEDULE, QW_INFO_LAST_K, QW_INFO_S
 # every symbol include/qw.h declares (tests/test_abi.py checks the header against this list)
 SYMBOLS = (
     "qw_create", "qw_create_batch", "qw_destroy", "qw_set_stream", "qw_set_lattice", "qw_set_coin",
-    "qw_set_site_phases", "qw_set_broken_links", "qw_set_state", "qw_set_state_delta", "qw_get_state",
+    "qw_set_site_phases", "qw_set_broken_links", "qw_set_random_broken_links", "qw_set_state", "qw_set_state_delta", "qw_get_state",
     "qw_step", "qw_step_inverse", "qw_probabilities", "qw_moments", "qw_set_schedule", "qw_set_window",
     "qw_get_info", "qw_synchronize", "qw_last_error",
 )
@@ -62,6 +62,7 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
         "qw_set_coin": [vp, ci, vp],
         "qw_set_site_phases": [vp, vp],
         "qw_set_broken_links": [vp, vp],
+        "qw_set_random_broken_links": [vp, ci, ctypes.c_double, ctypes.c_uint64],
         "qw_set_state": [vp, vp],
         "qw_set_state_delta": [vp, i64p, vp],
         "qw_get_state": [vp, vp],
@@ -149,6 +150,10 @@ def qw_set_site_phases(h, phases) -> None:
 
 def qw_set_broken_links(h, mask) -> None:
     _check(load().qw_set_broken_links(h, _ptr(mask)))
+
+
+def qw_set_random_broken_links(h, enable, p=0.0, seed=0) -> None:
+    _check(load().qw_set_random_broken_links(h, int(enable), float(p), int(seed)))
 
 
 def qw_set_state(h, amps) -> None:

@@ -273,6 +273,17 @@ int qw_set_broken_links(qw_sim *s, const uint8_t *mask) {
     return QW_OK;
 }
 
+int qw_set_random_broken_links(qw_sim *s, int enable, double p, uint64_t seed) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    if (!enable) { s->rbl = false; return QW_OK; }
+    if (!(p >= 0.0 && p <= 1.0)) return fail(QW_EINVAL, "the link-breaking probability must lie in [0, 1] (got %g)", p);
+    s->rbl = true;
+    s->rbl_seed = seed;
+    s->rbl_thr = (uint64_t)(p * 4294967296.0);   // floor(p * 2^32): a link is broken iff its 32-bit draw is below it
+    return QW_OK;
+}
+
 int qw_set_state(qw_sim *s, const void *amps) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
@@ -433,6 +444,9 @@ int qw_step_inverse(qw_sim *s, int64_t n) {
     if (n < 0) return fail(QW_EINVAL, "n must be >= 0 (got %lld)", (long long)n);
     if (!s->has_coin) return fail(QW_ESTATE, "qw_step_inverse before qw_set_coin");
     if (!s->has_state) return fail(QW_ESTATE, "qw_step_inverse before qw_set_state");
+    if (s->rbl && n > s->t)
+        return fail(QW_ESTATE, "with random broken links U(t) is defined for t >= 0 only: cannot take %lld inverse steps at t = %lld",
+                    (long long)n, s->t);
     for (int64_t i = 0; i < n; ++i) {
         int rc = launch_step_inverse(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur));
         if (rc) return rc;

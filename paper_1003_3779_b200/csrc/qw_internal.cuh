@@ -69,6 +69,9 @@ struct qw_sim {
     void *d_coin;            // PER_WALK / PER_SITE matrices on the device (handle dtype)
     void *d_phases;          // optional [batch][site] complex multipliers
     uint8_t *d_broken;       // optional [batch][site][coin] link mask
+    bool rbl;                // random broken links redrawn every step (qw_set_random_broken_links)
+    uint64_t rbl_seed;
+    uint64_t rbl_thr;        // floor(p * 2^32)
 
     // state bookkeeping
     bool has_state;

@@ -28,12 +28,47 @@ struct StepArgs {
     const typename Cx<R>::T *coins;
     const typename Cx<R>::T *phases;
     const uint8_t *broken;
+    // random broken links redrawn every step (qw_set_random_broken_links): a link is broken iff
+    // philox4x32_10(counter = (owner lo, owner hi, t, walk), key = seed)[axis] < rbl_thr
+    int rbl;
+    unsigned rbl_key0, rbl_key1;
+    unsigned long long rbl_thr;  // floor(p * 2^32), 0 .. 2^32
+    unsigned t;                  // step index (low 32 bits) of the U(t) being applied
     R coin[2 * CD * CD];
 };
 
 constexpr int STEP_BLOCK = 256;
 
-template <typename R, int DIM, int KIND, bool FAST, int U>
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, "Parallel random numbers: as easy as 1, 2, 3", SC'11), written from the
+// published round function.  Returns output word `axis` (0 or 1).
+__device__ __forceinline__ unsigned philox4x32_10_word(unsigned c0, unsigned c1, unsigned c2, unsigned c3,
+                                                       unsigned k0, unsigned k1, int axis) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const unsigned hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0; c1 = lo1; c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return axis == 0 ? c0 : c1;
+}
+
+// Is the link that component c of site (m,n) of walk w points along — it ends at (tm,tn) inside the lattice — broken
+// at step a.t?  The link is named by its OWNER (the end from which it points in the positive direction: dm > 0, or
+// dm = 0 and dn > 0) and its axis (0: along n / along (+1,+1); 1: along m / along (+1,-1)), so that both ends of a
+// link evaluate the same function and U(t) stays unitary (eq. 9: RBL is a property of the link).
+template <typename A>
+__device__ __forceinline__ bool rbl_link_broken(const A &a, long long w, long long m, long long n, long long tm,
+                                                long long tn, int dm, int dn) {
+    const bool positive = dm > 0 || (dm == 0 && dn > 0);
+    const unsigned long long owner = (unsigned long long)(positive ? (m * a.en + n) : (tm * a.en + tn));
+    const int axis = (dm != 0 && dn != 0) ? ((dm * dn > 0) ? 0 : 1) : (dm != 0 ? 1 : 0);
+    const unsigned word = philox4x32_10_word((unsigned)owner, (unsigned)(owner >> 32), a.t, (unsigned)w,
+                                             a.rbl_key0, a.rbl_key1, axis);
+    return (unsigned long long)word < a.rbl_thr;
+}
+
+template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false>
 __global__ void __launch_bounds__(STEP_BLOCK)
 step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
     constexpr int CD = 2 * DIM;
@@ -98,6 +133,9 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
             }
             if constexpr (!FAST) {
                 if (a.broken && a.broken[(w * a.sites + x) * CD + c]) stay = true;
+                if (a.rbl && !stay && rbl_link_broken(a, w, m, n, tm, tn, dm, dn)) stay = true;
+            } else if constexpr (RBL) {
+                if (!stay && rbl_link_broken(a, w, m, n, tm, tn, dm, dn)) stay = true;
             }
             const long long dst = stay ? ((CD - 1 - c) * a.plane_stride + row_off + n)
                                        : (c * a.plane_stride + w * a.walk_stride + tm * a.pitch + tn);
@@ -136,6 +174,7 @@ step_inverse_kernel(const StepArgs<R, 2 * DIM> a) {
             if (DIM == 2) stay |= (tm < 0) | (tm >= a.em);
         }
         if (a.broken && a.broken[(w * a.sites + x) * CD + c]) stay = true;
+        if (a.rbl && !stay && rbl_link_broken(a, w, m, n, tm, tn, dm, dn)) stay = true;
         const long long src = stay ? ((CD - 1 - c) * a.plane_stride + row_off + n)
                                    : (c * a.plane_stride + w * a.walk_stride + tm * a.pitch + tn);
         v[c] = cx_load<R>(a.in + src);
@@ -174,19 +213,37 @@ static void fill_args(const qw_sim *s, const void *in, void *out, const Box &box
     a.coins = static_cast<const V *>(s->d_coin);
     a.phases = static_cast<const V *>(s->d_phases);
     a.broken = s->d_broken;
+    a.rbl = s->rbl ? 1 : 0;
+    a.rbl_key0 = (unsigned)(s->rbl_seed & 0xffffffffu); a.rbl_key1 = (unsigned)(s->rbl_seed >> 32);
+    a.rbl_thr = s->rbl_thr;
+    a.t = (unsigned)((unsigned long long)s->t & 0xffffffffu);
     for (int i = 0; i < 2 * g.cdim * g.cdim; ++i) a.coin[i] = (R)s->h_coin[i];
 }
 
-template <typename R, int DIM, int KIND, bool FAST, int U>
+template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false>
 static int launch_scatter(qw_sim *s, StepArgs<R, 2 * DIM> &a) {
     const long long per_block = (long long)STEP_BLOCK * U;
     a.chunks_per_row = (int)((a.box_n + per_block - 1) / per_block);
     const long long blocks = s->g.batch * a.box_m * a.chunks_per_row;
     if (blocks <= 0) return QW_OK;
     if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
-    step_scatter_kernel<R, DIM, KIND, FAST, U><<<(unsigned)blocks, STEP_BLOCK, 0, s->stream>>>(a);
+    step_scatter_kernel<R, DIM, KIND, FAST, U, RBL><<<(unsigned)blocks, STEP_BLOCK, 0, s->stream>>>(a);
     QW_LAUNCH_CHECK(s, "step_scatter_kernel");
     return QW_OK;
+}
+
+template <typename R, int DIM, bool RBL>
+static int launch_fast_t(qw_sim *s, StepArgs<R, 2 * DIM> &a) {
+    // U sites per thread: 128 B of loads in flight per thread
+    constexpr int UF = (DIM == 1) ? (sizeof(R) == 8 ? 4 : 8) : (sizeof(R) == 8 ? 2 : 4);
+    switch (s->coin_kind) {
+        case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, true, UF, RBL>(s, a); break;
+        case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, true, UF, RBL>(s, a); break;
+        case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, true, UF, RBL>(s, a); break;
+        case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, true, UF, RBL>(s, a); break;
+        default: break;
+    }
+    return launch_scatter<R, DIM, COIN_GENERAL, true, UF, RBL>(s, a);
 }
 
 template <typename R, int DIM>
@@ -195,18 +252,7 @@ static int launch_step_t(qw_sim *s, const void *in, void *out, const Box &box, b
     fill_args<R, DIM>(s, in, out, box, a);
     const bool fast = allow_fast && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
                       s->g.lattice == QW_NATURAL;
-    // U sites per thread: 128 B of loads in flight per thread
-    constexpr int UF = (DIM == 1) ? (sizeof(R) == 8 ? 4 : 8) : (sizeof(R) == 8 ? 2 : 4);
-    if (fast) {
-        switch (s->coin_kind) {
-            case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, true, UF>(s, a); break;
-            case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, true, UF>(s, a); break;
-            case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, true, UF>(s, a); break;
-            case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, true, UF>(s, a); break;
-            default: break;
-        }
-        return launch_scatter<R, DIM, COIN_GENERAL, true, UF>(s, a);
-    }
+    if (fast) return s->rbl ? launch_fast_t<R, DIM, true>(s, a) : launch_fast_t<R, DIM, false>(s, a);
     // the general kernel keeps the coin kind of the uniform matrix so that schedules agree bit for bit
     if (s->coin_mode == QW_COIN_UNIFORM) {
         switch (s->coin_kind) {
@@ -233,6 +279,7 @@ static int launch_inverse_t(qw_sim *s, const void *in, void *out) {
     StepArgs<R, 2 * DIM> a;
     Box full{0, s->g.em - 1, 0, s->g.en - 1};
     fill_args<R, DIM>(s, in, out, full, a);
+    a.t = (unsigned)((unsigned long long)(s->t - 1) & 0xffffffffu);   // U(t-1)^dagger takes psi(t) back to psi(t-1)
     a.chunks_per_row = (int)((s->g.en + STEP_BLOCK - 1) / STEP_BLOCK);
     const long long blocks = s->g.batch * s->g.em * a.chunks_per_row;
     if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");

@@ -198,7 +198,7 @@ int blocked1d_granule(const qw_sim *s) {
 
 bool blocked1d_eligible(const qw_sim *s) {
     const Geom &g = s->g;
-    return g.dim == 1 && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
+    return g.dim == 1 && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken && !s->rbl &&
            g.en >= 32LL * blocked1d_granule(s);
 }
 

@@ -232,7 +232,7 @@ static int build_tmaps(qw_sim *s) {
 
 bool blocked2d_eligible(const qw_sim *s) {
     const Geom &g = s->g;
-    return g.dim == 2 && g.lattice == QW_NATURAL && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
+    return g.dim == 2 && g.lattice == QW_NATURAL && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken && !s->rbl &&
            g.em >= 2 * QW_GHOST_2D && g.en >= 2 * QW_GHOST_2D && g.batch <= 16383 && g.walk_stride * 4 * g.batch < (1LL << 40);
 }
 

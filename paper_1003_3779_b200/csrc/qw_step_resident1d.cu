@@ -205,7 +205,7 @@ step_resident1d_kernel(const Resident1dArgs<R> a) {
 
 bool resident1d_eligible(const qw_sim *s) {
     const Geom &g = s->g;
-    return g.dim == 1 && g.en <= RES_MAX_SITES && s->coin_mode != QW_COIN_PER_SITE && !s->d_broken &&
+    return g.dim == 1 && g.en <= RES_MAX_SITES && s->coin_mode != QW_COIN_PER_SITE && !s->d_broken && !s->rbl &&
            g.batch <= 0x7fffffffLL;
 }
 

@@ -1,0 +1,140 @@
+"""GPU parity for random broken links redrawn at every step (eqs. 9-10; R27):
+libqw evaluates the Philox4x32-10 link function inside its step kernels, the oracle evaluates its own copy
+of the published generator on the CPU; both must break exactly the same links at every step, so the states
+agree to the usual gates (complex128 1e-12, complex64 2e-5).  A single wrongly broken link moves O(|amp|)
+of amplitude, far above either gate.
+"""
+import numpy as np
+import pytest
+
+from paper_1003_3779_b200 import inputs as qi
+from test_parity_gpu import AMP_TOL, dev, small_workload  # noqa: F401  (dev is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+SEED = qi.SEED_RBL
+
+
+def gpu_rbl(qw, w, p, seed, steps, schedule=None, inverse=0, window=True, split=None):
+    h = qw.create_for(w)
+    try:
+        qw.qw_set_random_broken_links(h, 1, p, seed)
+        if schedule is not None:
+            qw.qw_set_schedule(h, schedule, 0)
+        qw.qw_set_window(h, window)
+        qw.load_state(h, w)
+        if split:
+            qw.qw_step(h, split)
+            qw.qw_step(h, steps - split)
+        else:
+            qw.qw_step(h, steps)
+        if inverse:
+            qw.qw_step_inverse(h, inverse)
+        amps = np.empty((w.batch, w.sites, w.coin_dim), dtype=w.dtype)
+        qw.qw_get_state(h, amps)
+        mom = np.empty((w.batch, 3 if w.dim == 1 else 6))
+        qw.qw_moments(h, mom)
+        return amps, mom, qw.qw_get_info(h, qw.QW_INFO_LAST_SCHEDULE), qw.qw_get_info(h, qw.QW_INFO_TIME)
+    finally:
+        qw.qw_destroy(h)
+
+
+def oracle_rbl(oracle, w, p, seed, steps, inverse=0):
+    mode, coin = w.general_coin_f64()
+    psi = np.ascontiguousarray(w.initial_state().astype(np.complex128))
+    kw = dict(boundary=w.boundary, coin_mode=mode, batch=w.batch, lattice=w.lattice)
+    oracle.step_rbl(w.extents, coin, psi, steps, p, seed, **kw)
+    if inverse:
+        oracle.step_inverse_rbl(w.extents, coin, psi, inverse, p, seed, t0=steps, **kw)
+    return psi
+
+
+def close(w, amps, psi):
+    d = float(np.max(np.abs(amps.astype(np.complex128) - psi)))
+    assert d <= AMP_TOL[np.dtype(w.dtype)], "max |d amplitude| = %.3e" % d
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("dim,lattice", [(1, qi.NATURAL), (2, qi.NATURAL), (2, qi.DIAGONAL)])
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+@pytest.mark.parametrize("p", [0.1, 0.5])
+def test_rbl_small_lattices_every_kernel(qw, oracle, dev, dtype, dim, lattice, boundary, p):
+    """Uniform random coin, batch of 2 (the walk index enters the counter): fused-RBL kernel where eligible
+    (natural lattice), generic kernel forced and for the diagonal lattice; same links => same state."""
+    rng = np.random.default_rng(41)
+    w = small_workload(dim, boundary, dtype, qi.COIN_UNIFORM, rng, lattice=lattice)
+    psi = oracle_rbl(oracle, w, p, SEED, 30)
+    a, mom, _, t = gpu_rbl(qw, w, p, SEED, 30)
+    close(w, a, psi)
+    assert t == 30
+    g, _, sched, _ = gpu_rbl(qw, w, p, SEED, 30, schedule=qw.QW_SCHED_GENERIC)
+    assert sched == qw.QW_SCHED_GENERIC
+    assert np.array_equal(a, g)                               # fused-RBL and generic kernels agree bit for bit
+    s, _, _, _ = gpu_rbl(qw, w, p, SEED, 30, split=11)        # the step index carries over between calls
+    assert np.array_equal(a, s)
+    if dtype == np.complex128:
+        assert np.max(np.abs(mom[:, 0] - 1)) < 1e-13          # every U(t) is unitary
+
+
+@pytest.mark.parametrize("coin_mode,phases", [(qi.COIN_PER_WALK, True), (qi.COIN_PER_SITE, False)])
+@pytest.mark.parametrize("dim", [1, 2])
+def test_rbl_with_coin_families(qw, oracle, dev, coin_mode, phases, dim):
+    rng = np.random.default_rng(42)
+    w = small_workload(dim, qi.OPEN, np.complex128, coin_mode, rng, phases=phases, batch=3)
+    close(w, gpu_rbl(qw, w, 0.3, 12345678901234567, 25)[0], oracle_rbl(oracle, w, 0.3, 12345678901234567, 25))
+
+
+@pytest.mark.parametrize("dim", [1, 2])
+def test_rbl_p0_and_p1_closed_forms(qw, oracle, dev, dim):
+    """p = 0: no link breaks => the plain walk, bit for bit.  p = 1: every link breaks => no amplitude ever
+    leaves its site (P(x) is conserved site by site)."""
+    rng = np.random.default_rng(43)
+    w = small_workload(dim, qi.PERIODIC, np.complex128, qi.COIN_UNIFORM, rng)
+    plain = np.ascontiguousarray(w.initial_state().astype(np.complex128))
+    oracle.step(w.extents, w.general_coin_f64()[1], plain, 12, boundary=w.boundary, batch=w.batch)
+    a0 = gpu_rbl(qw, w, 0.0, 7, 12)[0]
+    close(w, a0, plain)
+    a1 = gpu_rbl(qw, w, 1.0, 7, 12)[0]
+    P0 = np.sum(np.abs(w.initial_state()) ** 2, axis=-1)
+    assert np.max(np.abs(np.sum(np.abs(a1) ** 2, axis=-1) - P0)) < 1e-14
+    close(w, a1, oracle_rbl(oracle, w, 1.0, 7, 12))
+
+
+@pytest.mark.parametrize("dim,lattice", [(1, qi.NATURAL), (2, qi.NATURAL), (2, qi.DIAGONAL)])
+def test_rbl_inverse_undoes_the_same_link_sequence(qw, oracle, dev, dim, lattice):
+    rng = np.random.default_rng(44)
+    w = small_workload(dim, qi.OPEN, np.complex128, qi.COIN_UNIFORM, rng, lattice=lattice)
+    close(w, gpu_rbl(qw, w, 0.4, SEED, 20, inverse=7)[0], oracle_rbl(oracle, w, 0.4, SEED, 20, inverse=7))
+    back, _, _, t = gpu_rbl(qw, w, 0.4, SEED, 20, inverse=20)
+    assert t == 0
+    assert np.max(np.abs(back - w.initial_state())) <= 1e-13
+    h = qw.create_for(w)
+    try:
+        qw.qw_set_random_broken_links(h, 1, 0.4, SEED)
+        qw.load_state(h, w)
+        qw.qw_step(h, 3)
+        with pytest.raises(qw.QwError) as e:
+            qw.qw_step_inverse(h, 4)                             # would pass t = 0
+        assert e.value.code == qw.QW_ESTATE
+        with pytest.raises(qw.QwError) as e:
+            qw.qw_set_random_broken_links(h, 1, 1.5, 0)
+        assert e.value.code == qw.QW_EINVAL
+    finally:
+        qw.qw_destroy(h)
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+def test_rbl_multi_tile_lattices(qw, oracle, dev, dtype):
+    """Sizes that span several CTAs with ragged tails (owner indices cross block and row boundaries), the
+    named coins of PAPER.md:82, delta starts with the light-cone window (broken links only shrink the cone)."""
+    for w, p in ((qi.k1(sites=100003, steps=40, dtype=dtype), 0.05),
+                 (qi.k3(extents=(61, 1030), steps=24, coin="dft") if dtype == np.complex64
+                  else qi.k2(half=40, steps=60), 0.2),
+                 (qi.k4(batch=5, half=300, steps=200) if dtype == np.complex128
+                  else qi.k3(extents=(130, 97), steps=20, coin="hxh"), 0.1)):
+        psi = oracle_rbl(oracle, w, p, SEED, w.steps)
+        a, mom, _, _ = gpu_rbl(qw, w, p, SEED, w.steps)
+        close(w, a, psi)
+        if w.state is None:                                       # delta start: the window must not change anything
+            b = gpu_rbl(qw, w, p, SEED, w.steps, window=False)[0]
+            assert np.array_equal(a, b)
