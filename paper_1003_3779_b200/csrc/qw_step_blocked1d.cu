@@ -31,6 +31,7 @@ struct Blocked1dArgs {
     int valid;               // 32*M - 2k
     int boundary;
     R coin[8];
+    R scale_m;               // deferred-scale Hadamard: s^M, applied once per M steps (see blocked1d_step)
 };
 
 template <typename R> __device__ __forceinline__ cplx<R> shfl_up1(cplx<R> v) {
@@ -45,6 +46,14 @@ template <typename R> __device__ __forceinline__ cplx<R> shfl_down1(cplx<R> v) {
 }
 
 // One walk step with s = U (mod M).  x0 = unwrapped coordinate of this lane's logical site 0.
+//
+// Deferred scale (KIND == COIN_HADAMARD): the coin s*[[1,1],[1,-1]] is linear in s, so M consecutive steps equal
+// M unscaled butterflies (phi_R = R + L, phi_L = R - L: 4 additions per site-step instead of 2 mul + 4 fma)
+// followed by ONE multiplication by s^M.  Steps U = 0 .. M-2 run the bare butterfly, step U = M-1 runs the usual
+// scaled evaluation with s^M (C[1], filled by the launcher) in place of s.  The intermediate values grow by at most
+// 2^(M-1), far inside the exponent range, and are rescaled every M steps whatever the launch depth k, so the
+// result does not depend on k.  It differs from M scaled single steps by rounding only (fewer roundings, in fact):
+// <= 4 ulp per step (SURVEY.md 8(c) P13 "otherwise <= 4 ulp t").
 template <typename R, int M, int KIND, bool OPEN, int U>
 __device__ __forceinline__ void blocked1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
                                                bool wall_warp, long long x0, long long n_sites) {
@@ -52,7 +61,17 @@ __device__ __forceinline__ void blocked1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M
     for (int i = 0; i < M; ++i) {
         const int q = (i - U + M) % M, p = (i + U) % M;
         cplx<R> v[2] = {Rp[q], Lp[p]};
-        apply_coin<R, 2, KIND>(C, v);
+        if constexpr (KIND == COIN_HADAMARD) {
+            if constexpr (U + 1 < M) {
+                const cplx<R> r = v[0], l = v[1];
+                v[0] = cx_add(r, l);
+                v[1] = cx_sub(r, l);
+            } else {
+                apply_coin<R, 2, COIN_HADAMARD>(C + 1, v);      // C[1] = s^M
+            }
+        } else {
+            apply_coin<R, 2, KIND>(C, v);
+        }
         Rp[q] = v[0];
         Lp[p] = v[1];
     }
@@ -93,77 +112,163 @@ struct Blocked1dUnroll {
 // padded staging position of tile element e (row = owning lane): odd row length -> conflict-free
 template <int M> __device__ __forceinline__ int stage_pos(int e) { return (e / M) * (M + 1) + (e % M); }
 
+// 16- / 8-byte asynchronous global -> shared copy (LDGSTS); src_bytes = 0 writes zeros (sites outside an open lattice)
+template <int BYTES>
+__device__ __forceinline__ void cp_async_elem(void *smem_dst, const void *gmem_src, int src_bytes) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    if constexpr (BYTES == 16)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(gmem_src), "r"(src_bytes) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gmem_src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// resident CTAs per SM the kernel is sized for: 2 x 4 warps for complex128 (3 staging planes of 8.5 KB per warp
+// = 104 KB per CTA), 4 x 4 warps for complex64
+template <typename R> struct Blocked1dMinBlocks { static constexpr int value = sizeof(R) == 8 ? 2 : 4; };
+
+template <typename R, int M> constexpr size_t blocked1d_smem_bytes() {
+    return (size_t)BLK1D_WARPS * 3 * 32 * (M + 1) * sizeof(typename Cx<R>::T);
+}
+
+// Persistent warps: warp g of the grid walks over tiles g, g + G, g + 2G, ...  While tile n is advanced k steps in
+// registers, the input of tile n + G is already in flight (cp.async into the warp's two input planes of shared
+// memory), so the HBM round trip of a tile hides behind the arithmetic of the previous one instead of adding to it
+// (without the prefetch all resident warps load, compute and store in lock step: time = compute + memory).
 template <typename R, int M, int KIND, bool OPEN>
-__global__ void __launch_bounds__(BLK1D_WARPS * 32)
+__global__ void __launch_bounds__(BLK1D_WARPS * 32, Blocked1dMinBlocks<R>::value)
 step_blocked1d_kernel(const Blocked1dArgs<R> a) {
     typedef typename Cx<R>::T V;
-    __shared__ V stage[BLK1D_WARPS][32 * (M + 1)];
+    constexpr int PLANE = 32 * (M + 1);
+    extern __shared__ __align__(16) unsigned char blk1d_smem[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const long long tile_id = (long long)blockIdx.x * BLK1D_WARPS + wid;
-    if (tile_id >= a.total_tiles) return;          // whole warp exits together
-    const long long w = tile_id / a.tiles_per_walk;
-    const long long t = tile_id - w * a.tiles_per_walk;
+    V *st_in = reinterpret_cast<V *>(blk1d_smem) + (size_t)wid * 3 * PLANE;   // [2][PLANE]: prefetched input planes
+    V *st_out = st_in + 2 * PLANE;                                            // [PLANE]: output staging
     const long long N = a.n_sites;
-    const long long start = t * a.valid - a.k;     // unwrapped coordinate of tile element 0
-    const V *inw = a.in + w * a.walk_stride;
-    V *outw = a.out + w * a.walk_stride;
-    V *st = stage[wid];
+    const long long stride = (long long)gridDim.x * BLK1D_WARPS;
+    long long tile_id = (long long)blockIdx.x * BLK1D_WARPS + wid;
 
-    cplx<R> Rp[M], Lp[M];
-    // ---- load: coalesced global -> padded shared -> lane-contiguous registers, plane by plane
-#pragma unroll
-    for (int plane = 0; plane < 2; ++plane) {
-        V tmp[M];
-#pragma unroll
-        for (int i = 0; i < M; ++i) {
-            long long x = start + i * 32 + lane;
-            bool ok = true;
-            if (OPEN) ok = (x >= 0) && (x < N);
-            else { if (x < 0) x += N; else if (x >= N) x -= N; }
-            V z; z.x = 0; z.y = 0;
-            if (ok) z = inw[plane * a.plane_stride + x];
-            tmp[i] = z;
-        }
-#pragma unroll
-        for (int i = 0; i < M; ++i) st[stage_pos<M>(i * 32 + lane)] = tmp[i];
-        __syncwarp();
-#pragma unroll
-        for (int i = 0; i < M; ++i) {
-            const V z = st[lane * (M + 1) + i];
-            if (plane == 0) Rp[i] = cplx<R>{z.x, z.y}; else Lp[i] = cplx<R>{z.x, z.y};
-        }
-        __syncwarp();
-    }
+    // tile id -> (walk, tile of the walk); total_tiles < 2^31 (checked by the launcher)
+    auto split = [&](long long tid, long long &w, long long &t) {
+        if (a.tiles_per_walk == a.total_tiles) { w = 0; t = tid; return; }
+        const unsigned q = (unsigned)tid / (unsigned)a.tiles_per_walk;
+        w = q; t = (long long)((unsigned)tid - q * (unsigned)a.tiles_per_walk);
+    };
+    // element i*32 + lane of a tile sits at stage_pos(lane) + i * STEP_I of a staging plane (M divides 32)
+    constexpr int STEP_I = (32 / M) * (M + 1);
+    const int pos_lane = stage_pos<M>(lane);
 
-    // ---- k steps in registers
+    // coalesced global -> padded shared, both planes of one tile, asynchronously
+    auto prefetch = [&](long long tid) {
+        long long w, t;
+        split(tid, w, t);
+        const long long start = t * a.valid - a.k;
+        const V *inw = a.in + w * a.walk_stride;
+        if (start >= 0 && start + 32 * M <= N) {             // interior tile: no wrap, no wall -> immediate offsets only
+            const V *p0 = inw + start + lane, *p1 = p0 + a.plane_stride;
+            V *d0 = st_in + pos_lane, *d1 = d0 + PLANE;
+#pragma unroll
+            for (int i = 0; i < M; ++i) cp_async_elem<(int)sizeof(V)>(d0 + i * STEP_I, p0 + i * 32, (int)sizeof(V));
+#pragma unroll
+            for (int i = 0; i < M; ++i) cp_async_elem<(int)sizeof(V)>(d1 + i * STEP_I, p1 + i * 32, (int)sizeof(V));
+        } else {
+#pragma unroll 1
+            for (int plane = 0; plane < 2; ++plane) {
+#pragma unroll 4
+                for (int i = 0; i < M; ++i) {
+                    long long x = start + i * 32 + lane;
+                    bool ok = true;
+                    if (OPEN) ok = (x >= 0) && (x < N);
+                    else { if (x < 0) x += N; else if (x >= N) x -= N; }
+                    cp_async_elem<(int)sizeof(V)>(st_in + plane * PLANE + pos_lane + i * STEP_I,
+                                                  inw + plane * a.plane_stride + (ok ? x : 0), ok ? (int)sizeof(V) : 0);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+
     R C[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) C[i] = a.coin[i];
-    const long long x0 = start + (long long)lane * M;
-    bool wall_warp = false;
-    if (OPEN) wall_warp = (start <= 0) || (start + 32 * M >= N);
-    for (int s = 0; s < a.k; s += M)
-        Blocked1dUnroll<R, M, KIND, OPEN, 0>::run(Rp, Lp, C, wall_warp, x0, N);
+    if constexpr (KIND == COIN_HADAMARD) C[1] = a.scale_m;   // the imaginary part of C[0][0] (zero) is not used
 
-    // ---- store the valid middle: registers -> padded shared -> coalesced global
-#pragma unroll
-    for (int plane = 0; plane < 2; ++plane) {
-#pragma unroll
-        for (int i = 0; i < M; ++i) {
-            V z;
-            if (plane == 0) { z.x = Rp[i].re; z.y = Rp[i].im; } else { z.x = Lp[i].re; z.y = Lp[i].im; }
-            st[lane * (M + 1) + i] = z;
-        }
+    if (tile_id < a.total_tiles) prefetch(tile_id);
+    for (; tile_id < a.total_tiles; tile_id += stride) {
+        long long w, t;
+        split(tile_id, w, t);
+        const long long start = t * a.valid - a.k;     // unwrapped coordinate of tile element 0
+        V *outw = a.out + w * a.walk_stride;
+
+        // ---- padded shared -> lane-contiguous registers
+        cplx<R> Rp[M], Lp[M];
+        cp_async_wait_all();
         __syncwarp();
 #pragma unroll
         for (int i = 0; i < M; ++i) {
-            const int e = i * 32 + lane;
-            const long long xo = t * a.valid + (e - a.k);       // unwrapped output site
-            if (e >= a.k && e < 32 * M - a.k && xo < N)
-                outw[plane * a.plane_stride + xo] = st[stage_pos<M>(e)];
+            const V zr = st_in[lane * (M + 1) + i], zl = st_in[PLANE + lane * (M + 1) + i];
+            Rp[i] = cplx<R>{zr.x, zr.y};
+            Lp[i] = cplx<R>{zl.x, zl.y};
         }
         __syncwarp();
+        if (tile_id + stride < a.total_tiles) prefetch(tile_id + stride);
+
+        // ---- k steps in registers
+        const long long x0 = start + (long long)lane * M;
+        bool wall_warp = false;
+        if (OPEN) wall_warp = (start <= 0) || (start + 32 * M >= N);
+        for (int s = 0; s < a.k; s += M)
+            Blocked1dUnroll<R, M, KIND, OPEN, 0>::run(Rp, Lp, C, wall_warp, x0, N);
+
+        // ---- store the valid middle: registers -> padded shared -> coalesced global
+        const bool whole = (t + 1) * a.valid <= N;          // every valid output site of the tile is inside the lattice
+        const int lk = lane - a.k;                          // element e = i*32 + lane is valid iff 0 <= e - k < valid
+        V *o0 = outw + (t * a.valid + lk);
+#pragma unroll
+        for (int plane = 0; plane < 2; ++plane) {
+#pragma unroll
+            for (int i = 0; i < M; ++i) {
+                V z;
+                if (plane == 0) { z.x = Rp[i].re; z.y = Rp[i].im; } else { z.x = Lp[i].re; z.y = Lp[i].im; }
+                st_out[lane * (M + 1) + i] = z;
+            }
+            __syncwarp();
+            V *op = o0 + plane * a.plane_stride;
+            if (whole) {
+#pragma unroll
+                for (int i = 0; i < M; ++i)
+                    if ((unsigned)(lk + i * 32) < (unsigned)a.valid) op[i * 32] = st_out[pos_lane + i * STEP_I];
+            } else {
+#pragma unroll 4
+                for (int i = 0; i < M; ++i)
+                    if ((unsigned)(lk + i * 32) < (unsigned)a.valid && t * a.valid + lk + i * 32 < N)
+                        op[i * 32] = st_out[pos_lane + i * STEP_I];
+            }
+            __syncwarp();
+        }
     }
+}
+
+template <typename R, int M, int KIND, bool OPEN>
+static int launch_blocked1d_k(qw_sim *s, const Blocked1dArgs<R> &a) {
+    auto kern = step_blocked1d_kernel<R, M, KIND, OPEN>;
+    constexpr size_t smem = blocked1d_smem_bytes<R, M>();
+    static int ctas_per_sm = 0;      // per instantiation; the device is fixed for the life of the process' handles
+    if (ctas_per_sm == 0) {
+        QW_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int n = 0;
+        QW_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, BLK1D_WARPS * 32, smem));
+        if (n < 1) return fail(QW_ECUDA, "step_blocked1d_kernel does not fit on an SM (%zu bytes of shared memory)", smem);
+        ctas_per_sm = n;
+    }
+    if (a.total_tiles > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
+    long long blocks = (a.total_tiles + BLK1D_WARPS - 1) / BLK1D_WARPS;
+    const long long resident = (long long)s->sm_count * ctas_per_sm;
+    if (blocks > resident) blocks = resident;
+    kern<<<(unsigned)blocks, BLK1D_WARPS * 32, smem, s->stream>>>(a);
+    QW_LAUNCH_CHECK(s, "step_blocked1d_kernel");
+    return QW_OK;
 }
 
 template <typename R, int M, int KIND>
@@ -179,14 +284,11 @@ static int launch_blocked1d_t(qw_sim *s, const void *in, void *out, int k) {
     a.total_tiles = a.tiles_per_walk * g.batch;
     a.boundary = g.boundary;
     for (int i = 0; i < 8; ++i) a.coin[i] = (R)s->h_coin[i];
-    const long long blocks = (a.total_tiles + BLK1D_WARPS - 1) / BLK1D_WARPS;
-    if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
-    if (g.boundary == QW_OPEN)
-        step_blocked1d_kernel<R, M, KIND, true><<<(unsigned)blocks, BLK1D_WARPS * 32, 0, s->stream>>>(a);
-    else
-        step_blocked1d_kernel<R, M, KIND, false><<<(unsigned)blocks, BLK1D_WARPS * 32, 0, s->stream>>>(a);
-    QW_LAUNCH_CHECK(s, "step_blocked1d_kernel");
-    return QW_OK;
+    R sm = (R)1;
+    for (int i = 0; i < M; ++i) sm = (R)(sm * a.coin[0]);    // s^M by repeated rounded products in the handle's precision
+    a.scale_m = sm;
+    if (g.boundary == QW_OPEN) return launch_blocked1d_k<R, M, KIND, true>(s, a);
+    return launch_blocked1d_k<R, M, KIND, false>(s, a);
 }
 
 // Sites per lane: larger M = larger tiles (better valid fraction) but more registers and code.

@@ -217,7 +217,8 @@ def test_generic_and_fused_schedules_agree_bit_for_bit(qw, dev):
 @pytest.mark.parametrize("boundary", [qi.PERIODIC, qi.OPEN])
 @pytest.mark.parametrize("coin", ["hadamard", "su2"])
 def test_blocked_1d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, dtype, boundary, coin, ):
-    """P13: k steps per HBM round trip (warp-private register tiles) == k fused single steps, bit for bit;
+    """P13: k steps per HBM round trip (warp-private register tiles) == k fused single steps, bit for bit
+    (general coin) or to <= 4 ulp per step (Hadamard coin, whose scale is applied once per 16 steps);
     sizes span several tiles, a ragged last tile and the periodic seam / the reflecting walls."""
     rng = np.random.default_rng(3)
     for sites, steps, k, batch in ((5000, 96, 32, 1), (1031, 100, 16, 3), (70001, 131, 0, 1), (512, 48, 48, 2)):
@@ -227,9 +228,20 @@ def test_blocked_1d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, d
         a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
         b = gpu_run(qw, w, schedule=qw.QW_SCHED_BLOCKED, k=k)
         assert b[3]["sched"] == qw.QW_SCHED_BLOCKED and b[3]["launches"] < a[3]["launches"]
-        assert np.array_equal(a[0], b[0]), (sites, steps, k)
         auto = gpu_run(qw, w)
-        assert np.array_equal(a[0], auto[0])
+        if coin == "hadamard":
+            # deferred scale: 16 bare butterflies, then one multiplication by s^16 (qw_step_blocked1d.cu) -- equal to
+            # 16 scaled single steps up to rounding: <= 4 ulp per step; a wrong halo, seam or
+            # wall moves O(|amp|), ten orders above this bound
+            eps = np.finfo(np.float64 if dtype == np.complex128 else np.float32).eps
+            bound = 4 * eps * steps * float(np.max(np.abs(a[0])))
+            assert np.max(np.abs(a[0].astype(np.complex128) - b[0].astype(np.complex128))) <= bound, (sites, steps, k)
+            b16 = gpu_run(qw, w, schedule=qw.QW_SCHED_BLOCKED, k=16)
+            assert np.array_equal(b[0], b16[0]), "the launch depth k must not change the result"
+            assert np.array_equal(b16[0], auto[0]) or auto[3]["sched"] != qw.QW_SCHED_BLOCKED
+        else:
+            assert np.array_equal(a[0], b[0]), (sites, steps, k)
+            assert np.array_equal(a[0], auto[0])
     check_parity(w, b, oracle_run(oracle, w))
 
 
