@@ -1,6 +1,7 @@
 // qw_api.cu — the C ABI of include/qw.h: argument checking, device state ownership, host/device
 // pointer handling and the schedule dispatcher.  All arithmetic of the walk lives in the kernels
 // (qw_step*.cu, qw_reduce.cu); there is no CPU implementation of any step in this library.
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -49,8 +50,11 @@ static int classify_coin(const double *C, int cdim, int dtype) {
         if (real && sv != 0.0 && re(0, 1) == sv && re(1, 0) == sv && re(1, 1) == -sv) return COIN_HADAMARD;
         return COIN_GENERAL;
     }
+    // the 4x4 kinds require a power-of-two overall scale (1/2 for the unitary coins): the temporally blocked kernels
+    // defer it, which is exact only then (qw_coin.cuh: apply_coin_bare)
+    auto pow2 = [](double x) { int e; const double m = frexp(x < 0 ? -x : x, &e); return m == 0.5; };
     const double h = re(0, 0);
-    if (real && h != 0.0) {
+    if (real && h != 0.0 && pow2(h)) {
         static const int sgn[4][4] = {{1, 1, 1, 1}, {1, -1, 1, -1}, {1, 1, -1, -1}, {1, -1, -1, 1}};
         bool hxh = true;
         for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) if (re(a, b) != sgn[a][b] * h) hxh = false;
@@ -64,9 +68,9 @@ static int classify_coin(const double *C, int cdim, int dtype) {
         bool exact;
         if (dtype == QW_C64) { volatile float dg = (float)d - (float)g; volatile float back = dg + (float)g; exact = (back == (float)d); }
         else                 { volatile double dg = d - g; volatile double back = dg + g; exact = (back == d); }
-        if (gro && exact) return COIN_GROVER4;
+        if (gro && exact && g != 0.0 && pow2(g)) return COIN_GROVER4;
     }
-    if (h != 0.0 && im(0, 0) == 0.0) {
+    if (h != 0.0 && im(0, 0) == 0.0 && pow2(h)) {
         bool dft = true;
         for (int a = 0; a < 4; ++a) for (int b = 0; b < 4; ++b) {
             const int p = (a * b) & 3;

@@ -126,6 +126,39 @@ __device__ __forceinline__ void apply_coin(const R *__restrict__ C, cplx<R> (&v)
     }
 }
 
+// The named 4x4 coins WITHOUT their overall scale (temporally blocked kernels defer it): the host only classifies a
+// matrix as Grover / H(x)H / DFT when that scale (g resp. h) is a power of two, so that multiplying by it commutes
+// with every rounding: K bare steps followed by one multiplication by scale^K give bit for bit the state of K
+// scaled steps (no overflow: the bare values grow by at most 4^K; underflow to denormals aside).
+//   Grover-like  g*sum + (d-g)*psi_a  = g * (sum + r*psi_a),  r = (d-g)/g  (= -2 for the Grover coin)
+//   H(x)H, DFT   the radix-2 butterflies of apply_coin with h = 1
+template <typename R, int KIND>
+__device__ __forceinline__ void apply_coin_bare(R r, cplx<R> (&v)[4]) {
+    static_assert(KIND == COIN_GROVER4 || KIND == COIN_HXH4 || KIND == COIN_DFT4, "no bare form for this coin");
+    if constexpr (KIND == COIN_GROVER4) {
+        const cplx<R> sum = cx_add(cx_add(v[0], v[1]), cx_add(v[2], v[3]));
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            v[a].re = fma_rn(r, v[a].re, sum.re);
+            v[a].im = fma_rn(r, v[a].im, sum.im);
+        }
+    } else if constexpr (KIND == COIN_HXH4) {
+        const cplx<R> a0 = cx_add(v[0], v[1]), a1 = cx_sub(v[0], v[1]);
+        const cplx<R> a2 = cx_add(v[2], v[3]), a3 = cx_sub(v[2], v[3]);
+        v[0] = cx_add(a0, a2);
+        v[1] = cx_add(a1, a3);
+        v[2] = cx_sub(a0, a2);
+        v[3] = cx_sub(a1, a3);
+    } else {
+        const cplx<R> e0 = cx_add(v[0], v[2]), e1 = cx_sub(v[0], v[2]);
+        const cplx<R> o0 = cx_add(v[1], v[3]), o1 = cx_muli(cx_sub(v[1], v[3]));
+        v[0] = cx_add(e0, o0);
+        v[1] = cx_add(e1, o1);
+        v[2] = cx_sub(e0, o0);
+        v[3] = cx_sub(e1, o1);
+    }
+}
+
 // psi = C^dagger phi in place (inverse step; general evaluation only).
 template <typename R, int CD>
 __device__ __forceinline__ void apply_coin_dagger(const R *__restrict__ C, cplx<R> (&v)[CD]) {

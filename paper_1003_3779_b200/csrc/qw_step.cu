@@ -38,6 +38,12 @@ struct StepArgs {
 };
 
 constexpr int STEP_BLOCK = 256;
+// Launch shape of the fused kernel, measured on B200 (profiles/r01_fused_step.md, "launch shapes"):
+// threads per block BS and sites per thread U (strided by the block).
+template <typename R, int DIM> struct FusedShape {
+    static constexpr int BS = (DIM == 2 && sizeof(R) == 4) ? 128 : 256;
+    static constexpr int U = (DIM == 1) ? (sizeof(R) == 8 ? 4 : 8) : (sizeof(R) == 8 ? 1 : 4);
+};
 
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, "Parallel random numbers: as easy as 1, 2, 3", SC'11), written from the
 // published round function.  Returns output word `axis` (0 or 1).
@@ -68,8 +74,8 @@ __device__ __forceinline__ bool rbl_link_broken(const A &a, long long w, long lo
     return (unsigned long long)word < a.rbl_thr;
 }
 
-template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false>
-__global__ void __launch_bounds__(STEP_BLOCK)
+template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK>
+__global__ void __launch_bounds__(BS)
 step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
     constexpr int CD = 2 * DIM;
     typedef typename Cx<R>::T V;
@@ -79,14 +85,14 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
     const int chunk = (int)(blk - rowid * a.chunks_per_row);
     const long long w = rowid / a.box_m;
     const long long m = a.m_lo + (rowid - w * a.box_m);
-    const long long n_base = (long long)chunk * (STEP_BLOCK * U) + threadIdx.x;
+    const long long n_base = (long long)chunk * (BS * U) + threadIdx.x;
     const long long row_off = w * a.walk_stride + m * a.pitch;
 
     cplx<R> v[U][CD];
     bool live[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
-        const long long nb = n_base + (long long)u * STEP_BLOCK;
+        const long long nb = n_base + (long long)u * BS;
         live[u] = nb < a.box_n;
         if (live[u]) {
             const long long idx = row_off + a.n_lo + nb;
@@ -97,7 +103,7 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         if (!live[u]) continue;
-        const long long n = a.n_lo + n_base + (long long)u * STEP_BLOCK;
+        const long long n = a.n_lo + n_base + (long long)u * BS;
         const long long x = m * a.en + n;
         if constexpr (FAST) {
             apply_coin<R, CD, KIND>(a.coin, v[u]);
@@ -220,30 +226,29 @@ static void fill_args(const qw_sim *s, const void *in, void *out, const Box &box
     for (int i = 0; i < 2 * g.cdim * g.cdim; ++i) a.coin[i] = (R)s->h_coin[i];
 }
 
-template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false>
+template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK>
 static int launch_scatter(qw_sim *s, StepArgs<R, 2 * DIM> &a) {
-    const long long per_block = (long long)STEP_BLOCK * U;
+    const long long per_block = (long long)BS * U;
     a.chunks_per_row = (int)((a.box_n + per_block - 1) / per_block);
     const long long blocks = s->g.batch * a.box_m * a.chunks_per_row;
     if (blocks <= 0) return QW_OK;
     if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
-    step_scatter_kernel<R, DIM, KIND, FAST, U, RBL><<<(unsigned)blocks, STEP_BLOCK, 0, s->stream>>>(a);
+    step_scatter_kernel<R, DIM, KIND, FAST, U, RBL, BS><<<(unsigned)blocks, BS, 0, s->stream>>>(a);
     QW_LAUNCH_CHECK(s, "step_scatter_kernel");
     return QW_OK;
 }
 
 template <typename R, int DIM, bool RBL>
 static int launch_fast_t(qw_sim *s, StepArgs<R, 2 * DIM> &a) {
-    // U sites per thread: 128 B of loads in flight per thread
-    constexpr int UF = (DIM == 1) ? (sizeof(R) == 8 ? 4 : 8) : (sizeof(R) == 8 ? 2 : 4);
+    constexpr int UF = FusedShape<R, DIM>::U, BS = FusedShape<R, DIM>::BS;
     switch (s->coin_kind) {
-        case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, true, UF, RBL>(s, a); break;
-        case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, true, UF, RBL>(s, a); break;
-        case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, true, UF, RBL>(s, a); break;
-        case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, true, UF, RBL>(s, a); break;
+        case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, true, UF, RBL, BS>(s, a); break;
+        case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, true, UF, RBL, BS>(s, a); break;
+        case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, true, UF, RBL, BS>(s, a); break;
+        case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, true, UF, RBL, BS>(s, a); break;
         default: break;
     }
-    return launch_scatter<R, DIM, COIN_GENERAL, true, UF, RBL>(s, a);
+    return launch_scatter<R, DIM, COIN_GENERAL, true, UF, RBL, BS>(s, a);
 }
 
 template <typename R, int DIM>

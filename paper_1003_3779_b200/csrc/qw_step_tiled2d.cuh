@@ -47,6 +47,10 @@ struct Tiled2dArgs {
     int tile_m0, tile_n0;         // first tile (of the global tile grid) of the launched range
     int tiles_m, tiles_n;         // extent of the launched range
     R coin[32];
+    // deferred scale of the named coins (qw_coin.cuh: apply_coin_bare): steps 0 .. K-2 run the bare coin, step K-1
+    // the scaled evaluation with coin_last = coin * scale^(K-1) (an exact power-of-two multiple)
+    R coin_last[32];
+    R ratio;                      // Grover-like: (d - g) / g
 };
 
 __host__ __device__ constexpr int t2d_mod(int a, int m) { return ((a % m) + m) % m; }
@@ -130,9 +134,9 @@ struct Walls {
 // xb = exchange slots of this step's parity: V xb[W][2][RN][32]; xbar = their W "slot of warp w is full"
 // mbarriers; bit (S & 1) of xph = the phase parity to wait for.  A warp only waits for its two neighbours:
 // they can never be more than one step apart, so the double-buffered slots and barriers are race-free.
-template <typename R, int RM, int RN, int W, int KIND, bool OPEN, int S>
-__device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename Cx<R>::T *xb, uint64_t *xbar, uint32_t &xph,
-                                     int lane, int wid, bool wall_tile, const Walls &wl) {
+template <typename R, int RM, int RN, int W, int KIND, bool OPEN, int S, bool LAST>
+__device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, const R *Clast, R ratio, typename Cx<R>::T *xb,
+                                     uint64_t *xbar, uint32_t &xph, int lane, int wid, bool wall_tile, const Walls &wl) {
     typedef typename Cx<R>::T V;
     // ---- coin (eq. 1) on every site of the patch, in place
 #pragma unroll
@@ -141,7 +145,9 @@ __device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename C
         for (int j = 0; j < RN; ++j) {
             cplx<R> v[4] = {p.c0[i][t2d_mod(j - S, RN)], p.c1[t2d_mod(i - S, RM)][j],
                             p.c2[t2d_mod(i + S, RM)][j], p.c3[i][t2d_mod(j + S, RN)]};
-            apply_coin<R, 4, KIND>(C, v);
+            if constexpr (KIND == COIN_GENERAL) apply_coin<R, 4, KIND>(C, v);
+            else if constexpr (LAST) apply_coin<R, 4, KIND>(Clast, v);
+            else apply_coin_bare<R, KIND>(ratio, v);
             p.c0[i][t2d_mod(j - S, RN)] = v[0];
             p.c1[t2d_mod(i - S, RM)][j] = v[1];
             p.c2[t2d_mod(i + S, RM)][j] = v[2];
@@ -248,10 +254,12 @@ __device__ __forceinline__ void step(Patch<R, RM, RN> &p, const R *C, typename C
 
 template <typename R, int RM, int RN, int W, int KIND, bool OPEN, int S, int K>
 struct Steps {
-    static __device__ __forceinline__ void run(Patch<R, RM, RN> &p, const R *C, typename Cx<R>::T *xch, uint64_t *xbar,
-                                               uint32_t &xph, int lane, int wid, bool wall_tile, const Walls &wl) {
-        step<R, RM, RN, W, KIND, OPEN, S>(p, C, xch + (S & 1) * (W * 2 * RN * 32), xbar + (S & 1) * W, xph, lane, wid, wall_tile, wl);
-        if constexpr (S + 1 < K) Steps<R, RM, RN, W, KIND, OPEN, S + 1, K>::run(p, C, xch, xbar, xph, lane, wid, wall_tile, wl);
+    static __device__ __forceinline__ void run(Patch<R, RM, RN> &p, const R *C, const R *Clast, R ratio, typename Cx<R>::T *xch,
+                                               uint64_t *xbar, uint32_t &xph, int lane, int wid, bool wall_tile, const Walls &wl) {
+        step<R, RM, RN, W, KIND, OPEN, S, S + 1 == K>(p, C, Clast, ratio, xch + (S & 1) * (W * 2 * RN * 32), xbar + (S & 1) * W, xph,
+                                                      lane, wid, wall_tile, wl);
+        if constexpr (S + 1 < K)
+            Steps<R, RM, RN, W, KIND, OPEN, S + 1, K>::run(p, C, Clast, ratio, xch, xbar, xph, lane, wid, wall_tile, wl);
     }
 };
 
@@ -342,7 +350,7 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
             wl.jl = (jl >= 0 && jl < RN) ? (int)jl : -1;
             wl.jr = (jr >= 0 && jr < RN) ? (int)jr : -1;
         }
-        t2d::Steps<R, RM, RN, W, KIND, OPEN, 0, K>::run(p, C, xch, xbar, xph, lane, wid, wall_tile, wl);
+        t2d::Steps<R, RM, RN, W, KIND, OPEN, 0, K>::run(p, C, a.coin_last, a.ratio, xch, xbar, xph, lane, wid, wall_tile, wl);
 
         // ---- store the valid interior straight from registers: psi_c(i, j) after K steps sits at
         //      c0[i][(j-K) mod RN], c1[(i-K) mod RM][j], c2[(i+K) mod RM][j], c3[i][(j+K) mod RN]

@@ -60,6 +60,12 @@ static int t2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     a.tiles_m = (int)(box.m_hi / TM) - a.tile_m0 + 1; a.tiles_n = (int)(box.n_hi / TN) - a.tile_n0 + 1;
     a.total_tiles = (long long)a.tiles_m * a.tiles_n * g.batch;
     for (int i = 0; i < 32; ++i) a.coin[i] = (R)s->h_coin[i];
+    // deferred scale (named coins only; their scale is a power of two, so every product below is exact)
+    const double scale = KIND == COIN_GROVER4 ? s->h_coin[2] : s->h_coin[0];
+    double pw = 1.0;
+    for (int i = 0; i < K - 1; ++i) pw *= scale;
+    for (int i = 0; i < 32; ++i) a.coin_last[i] = (R)(s->h_coin[i] * pw);
+    a.ratio = KIND == COIN_GROVER4 ? (R)((s->h_coin[0] - s->h_coin[2]) / s->h_coin[2]) : (R)0;
     const size_t smem = tiled2d_smem_bytes<R>();
     const long long cap = (long long)s->sm_count;              // persistent: one CTA per SM
     const unsigned grid = (unsigned)(a.total_tiles < cap ? a.total_tiles : cap);
