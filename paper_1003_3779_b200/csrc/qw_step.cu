@@ -7,7 +7,7 @@
 //
 // Two instantiation families share the code:
 //   FAST    uniform coin held in the kernel parameters (constant bank), no phases, no link
-//           mask, natural lattice; U sites per thread, strided by the block so that every warp
+//           mask; natural or diagonal lattice, optional random broken links; U sites per thread, strided by the block so that every warp
 //           access is one contiguous run                       -> QW_SCHED_FUSED
 //   GENERAL every feature decided at run time (per-walk / per-site coins, phases, broken links,
 //           diagonal lattice)                                  -> QW_SCHED_GENERIC
@@ -74,7 +74,7 @@ __device__ __forceinline__ bool rbl_link_broken(const A &a, long long w, long lo
     return (unsigned long long)word < a.rbl_thr;
 }
 
-template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK>
+template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK, bool DIAG = false>
 __global__ void __launch_bounds__(BS)
 step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
     constexpr int CD = 2 * DIM;
@@ -127,7 +127,7 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
 #pragma unroll
         for (int c = 0; c < CD; ++c) {
             int dm, dn;
-            coin_direction<DIM>(FAST ? QW_NATURAL : a.lattice, c, dm, dn);
+            coin_direction<DIM>(FAST ? (DIAG ? QW_DIAGONAL : QW_NATURAL) : a.lattice, c, dm, dn);
             long long tm = m + dm, tn = n + dn;
             bool stay = false;
             if (a.boundary == QW_PERIODIC) {
@@ -226,38 +226,43 @@ static void fill_args(const qw_sim *s, const void *in, void *out, const Box &box
     for (int i = 0; i < 2 * g.cdim * g.cdim; ++i) a.coin[i] = (R)s->h_coin[i];
 }
 
-template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK>
+template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK, bool DIAG = false>
 static int launch_scatter(qw_sim *s, StepArgs<R, 2 * DIM> &a) {
     const long long per_block = (long long)BS * U;
     a.chunks_per_row = (int)((a.box_n + per_block - 1) / per_block);
     const long long blocks = s->g.batch * a.box_m * a.chunks_per_row;
     if (blocks <= 0) return QW_OK;
     if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
-    step_scatter_kernel<R, DIM, KIND, FAST, U, RBL, BS><<<(unsigned)blocks, BS, 0, s->stream>>>(a);
+    step_scatter_kernel<R, DIM, KIND, FAST, U, RBL, BS, DIAG><<<(unsigned)blocks, BS, 0, s->stream>>>(a);
     QW_LAUNCH_CHECK(s, "step_scatter_kernel");
     return QW_OK;
 }
 
-template <typename R, int DIM, bool RBL>
+template <typename R, int DIM, bool RBL, bool DIAG>
 static int launch_fast_t(qw_sim *s, StepArgs<R, 2 * DIM> &a) {
     constexpr int UF = FusedShape<R, DIM>::U, BS = FusedShape<R, DIM>::BS;
     switch (s->coin_kind) {
-        case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, true, UF, RBL, BS>(s, a); break;
-        case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, true, UF, RBL, BS>(s, a); break;
-        case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, true, UF, RBL, BS>(s, a); break;
-        case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, true, UF, RBL, BS>(s, a); break;
+        case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, true, UF, RBL, BS, DIAG>(s, a); break;
+        case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, true, UF, RBL, BS, DIAG>(s, a); break;
+        case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, true, UF, RBL, BS, DIAG>(s, a); break;
+        case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, true, UF, RBL, BS, DIAG>(s, a); break;
         default: break;
     }
-    return launch_scatter<R, DIM, COIN_GENERAL, true, UF, RBL, BS>(s, a);
+    return launch_scatter<R, DIM, COIN_GENERAL, true, UF, RBL, BS, DIAG>(s, a);
 }
 
 template <typename R, int DIM>
 static int launch_step_t(qw_sim *s, const void *in, void *out, const Box &box, bool allow_fast) {
     StepArgs<R, 2 * DIM> a;
     fill_args<R, DIM>(s, in, out, box, a);
-    const bool fast = allow_fast && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
-                      s->g.lattice == QW_NATURAL;
-    if (fast) return s->rbl ? launch_fast_t<R, DIM, true>(s, a) : launch_fast_t<R, DIM, false>(s, a);
+    const bool fast = allow_fast && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken;
+    if (fast) {
+        if constexpr (DIM == 2) {
+            if (s->g.lattice == QW_DIAGONAL)
+                return s->rbl ? launch_fast_t<R, DIM, true, true>(s, a) : launch_fast_t<R, DIM, false, true>(s, a);
+        }
+        return s->rbl ? launch_fast_t<R, DIM, true, false>(s, a) : launch_fast_t<R, DIM, false, false>(s, a);
+    }
     // the general kernel keeps the coin kind of the uniform matrix so that schedules agree bit for bit
     if (s->coin_mode == QW_COIN_UNIFORM) {
         switch (s->coin_kind) {

@@ -170,6 +170,30 @@ def test_diagonal_lattice(qw, oracle, dev, boundary, dtype):
     check_parity(w, gpu_run(qw, w), oracle_run(oracle, w))
 
 
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("coin", ["hxh", "dft", "grover"])
+def test_diagonal_lattice_fused_path_multi_tile(qw, oracle, dev, boundary, dtype, coin):
+    """The lattice of the paper's Tables 2-3 (Fig. 1c :106) through the vectorised fused kernel:
+    several CTAs per row with ragged tails, named coins, random state and a delta start whose light-cone window
+    reaches the walls; fused == generic bit for bit."""
+    w = qi.k3(extents=(37, 1100), steps=21, coin=coin, dtype=dtype)
+    w.lattice, w.boundary = qi.DIAGONAL, boundary
+    a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+    g = gpu_run(qw, w, schedule=qw.QW_SCHED_GENERIC)
+    assert a[3]["sched"] == qw.QW_SCHED_FUSED and np.array_equal(a[0], g[0])
+    assert np.array_equal(a[0], gpu_run(qw, w)[0])                      # AUTO picks a kernel that knows the lattice
+    check_parity(w, a, oracle_run(oracle, w))
+    d = qi.k2(half=30, steps=45)
+    d.lattice, d.boundary = qi.DIAGONAL, boundary
+    d.dtype = np.dtype(dtype); d.coin = {"hxh": qi.hadamard_x_hadamard, "dft": qi.dft4, "grover": qi.grover4}[coin](dtype)
+    d.delta_coin = d.delta_coin.astype(dtype)
+    on = gpu_run(qw, d, window=True)
+    off = gpu_run(qw, d, window=False)
+    assert np.array_equal(on[0], off[0])
+    check_parity(d, on, oracle_run(oracle, d))
+
+
 @pytest.mark.parametrize("dim,lattice", [(1, qi.NATURAL), (2, qi.NATURAL), (2, qi.DIAGONAL)])
 @pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
 def test_static_broken_links(qw, oracle, dev, dim, lattice, boundary):
