@@ -90,13 +90,20 @@ def coin_cost(w, sched_name="fused"):
         if w.phases is not None:
             instr, flops = instr + 8, flops + 12
         return instr, flops
+    # 2D named coins: scaled evaluation 20 / 16 / 20 instructions; the tiled kernel defers the power-of-two scale:
+    # K-1 bare steps (H(x)H, DFT: 16 add; Grover: 6 add + 8 fma) + 1 scaled step per K steps
+    K = 8 if w.dtype == np.complex64 else 6
+    def tiled(bare_i, bare_f, full_i, full_f):
+        if sched_name == "tiled":
+            return ((K - 1) * bare_i + full_i) / K, ((K - 1) * bare_f + full_f) / K
+        return full_i, full_f
     if w.coin_mode == qi.COIN_UNIFORM and np.all(c.imag == 0) and np.all(np.abs(c) == abs(c[0, 0])):
         if np.array_equal(np.sign(c.real), np.sign(qi.hadamard_x_hadamard().real)):
-            return 20, 24          # 2 mul + 4 fma + 4 add per real component; 16 add + 8 mul algorithmic
+            return tiled(16, 16, 20, 24)      # scaled: 2 mul + 4 fma + 4 add per real component
     if w.coin_mode == qi.COIN_UNIFORM and np.array_equal(c, qi.grover4(c.dtype)):
-        return 16, 24
+        return tiled(14, 22, 16, 24)
     if w.coin_mode == qi.COIN_UNIFORM and np.array_equal(c, qi.dft4(c.dtype)):
-        return 20, 24
+        return tiled(16, 16, 20, 24)
     return 64, 120
 
 

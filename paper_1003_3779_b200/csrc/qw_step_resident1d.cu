@@ -77,7 +77,7 @@ __device__ __forceinline__ void resident_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M]
             cplx<R> v[2] = {Rp[q], Lp[p]};
             apply_coin<R, 2, KIND>(C, v);
             if constexpr (PHASES) {
-                const cplx<R> ph = from_v<R>(cx.ph[cx.tid * (M + 1) + i]);
+                const cplx<R> ph = from_v<R>(cx.ph[cx.tid * (M | 1) + i]);
                 v[0] = cx_mul(ph.re, ph.im, v[0]);
                 v[1] = cx_mul(ph.re, ph.im, v[1]);
             }
@@ -157,7 +157,7 @@ step_resident1d_kernel(const Resident1dArgs<R> a) {
         for (long long e = tid; e < (long long)blockDim.x * M; e += blockDim.x) {
             V z; z.x = 0; z.y = 0;
             if (e < N) z = a.phases[w * N + e];
-            ph[(e / M) * (M + 1) + (e % M)] = z;
+            ph[(e / M) * (M | 1) + (e % M)] = z;       // odd row length: conflict-free 16-byte reads
         }
     }
     R C[8];
@@ -226,7 +226,7 @@ static int launch_resident_shape(qw_sim *s, const void *in, void *out, long long
     int threads = (int)((g.en + M - 1) / M);
     threads = (threads + 31) / 32 * 32;
     const int nw = threads / 32;
-    const size_t smem = sizeof(V) * (size_t)(4 * nw + 4 + (PHASES ? (size_t)threads * (M + 1) : 0));
+    const size_t smem = sizeof(V) * (size_t)(4 * nw + 4 + (PHASES ? (size_t)threads * (M | 1) : 0));
     auto launch = [&](auto kernel) -> int {
         if (smem > 48 * 1024)
             QW_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
