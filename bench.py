@@ -353,6 +353,9 @@ def run_gpu(args):
         qw.qw_set_schedule(h, {"auto": 0, "generic": 1, "fused": 2, "blocked": 3, "resident": 4, "tiled": 5}[args.schedule], args.k)
     if args.no_window:
         qw.qw_set_window(h, 0)
+    if args.rbl is not None:
+        # NEXT-2: every link redrawn broken with probability p at every step (eqs. 9-10)
+        qw.qw_set_random_broken_links(h, 1, args.rbl, qi.SEED_RBL)
     stream = torch.cuda.current_stream()
     qw.qw_set_stream(h, stream.cuda_stream)
 
@@ -513,7 +516,8 @@ def run_gpu(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f64" if w.dtype == np.complex128 else "f32",
         "data": "synthetic",
         "config": workload_config(args.workload, w, {"schedule": sched_name, "k": kdepth, "window": bool(windowed),
-                                                     "step_ms": step_ms / args.steps, "outputs_ms": out_ms / args.steps}),
+                                                     "step_ms": step_ms / args.steps, "outputs_ms": out_ms / args.steps,
+                                                     **({"random_broken_links_p": args.rbl} if args.rbl is not None else {})}),
         "effective_hbm_gbs": eff_gbs,
         "roofline": roofline,
         "fused_single_step": fused,
@@ -541,6 +545,7 @@ def main():
     ap.add_argument("--schedule", default=None, choices=["auto", "generic", "fused", "blocked", "resident", "tiled"])
     ap.add_argument("--k", type=int, default=0)
     ap.add_argument("--no-window", action="store_true")
+    ap.add_argument("--rbl", type=float, default=None, help="random broken links redrawn every step with this probability")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fused-leg", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -372,7 +372,7 @@ int qw_step(qw_sim *s, int64_t n) {
     int sched = s->sched;
     if (sched == QW_SCHED_AUTO)
         sched = resident1d_eligible(s) ? QW_SCHED_RESIDENT
-              : (blocked1d_eligible(s) && n >= blocked1d_granule(s)) ? QW_SCHED_BLOCKED
+              : (blocked1d_eligible(s) && n >= 4) ? QW_SCHED_BLOCKED
               : (tiled2d_eligible(s) && n >= 2) ? QW_SCHED_TILED : QW_SCHED_FUSED;
     if (sched == QW_SCHED_RESIDENT) {
         if (!resident1d_eligible(s))
@@ -425,8 +425,10 @@ int qw_step(qw_sim *s, int64_t n) {
         kmax = kmax / M * M;
         if (kmax < M) kmax = M;
         s->last_k = kmax;
-        while (remaining >= M) {
-            const int kk = (int)(remaining >= kmax ? kmax : remaining / M * M);
+        // multiples of M with the big tiles, then a remainder of 4 .. 15 steps with short 8- / 4-step launches (small
+        // tiles, the fused kernel's arithmetic), then at most 3 fused single steps
+        while (remaining >= 4) {
+            const int kk = remaining >= M ? (int)(remaining >= kmax ? kmax : remaining / M * M) : (remaining >= 8 ? 8 : 4);
             int rc = launch_step_blocked1d(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), kk);
             if (rc) return rc;
             s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;

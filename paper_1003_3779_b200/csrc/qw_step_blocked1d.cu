@@ -47,7 +47,8 @@ template <typename R> __device__ __forceinline__ cplx<R> shfl_down1(cplx<R> v) {
 
 // One walk step with s = U (mod M).  x0 = unwrapped coordinate of this lane's logical site 0.
 //
-// Deferred scale (KIND == COIN_HADAMARD): the coin s*[[1,1],[1,-1]] is linear in s, so M consecutive steps equal
+// Deferred scale (KIND == COIN_HADAMARD with M = 16; the short M = 8 / M = 4 tiles that mop up a remainder of 4 .. 15
+// steps use the scaled evaluation of the fused kernel, bit for bit): the coin s*[[1,1],[1,-1]] is linear in s, so M consecutive steps equal
 // M unscaled butterflies (phi_R = R + L, phi_L = R - L: 4 additions per site-step instead of 2 mul + 4 fma)
 // followed by ONE multiplication by s^M.  Steps U = 0 .. M-2 run the bare butterfly, step U = M-1 runs the usual
 // scaled evaluation with s^M (C[1], filled by the launcher) in place of s.  The intermediate values grow by at most
@@ -61,7 +62,7 @@ __device__ __forceinline__ void blocked1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M
     for (int i = 0; i < M; ++i) {
         const int q = (i - U + M) % M, p = (i + U) % M;
         cplx<R> v[2] = {Rp[q], Lp[p]};
-        if constexpr (KIND == COIN_HADAMARD) {
+        if constexpr (KIND == COIN_HADAMARD && M == 16) {
             if constexpr (U + 1 < M) {
                 const cplx<R> r = v[0], l = v[1];
                 v[0] = cx_add(r, l);
@@ -192,7 +193,7 @@ step_blocked1d_kernel(const Blocked1dArgs<R> a) {
     R C[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) C[i] = a.coin[i];
-    if constexpr (KIND == COIN_HADAMARD) C[1] = a.scale_m;   // the imaginary part of C[0][0] (zero) is not used
+    if constexpr (KIND == COIN_HADAMARD && M == 16) C[1] = a.scale_m;   // the imaginary part of C[0][0] (zero) is not used
 
     if (tile_id < a.total_tiles) prefetch(tile_id);
     for (; tile_id < a.total_tiles; tile_id += stride) {
@@ -291,9 +292,9 @@ static int launch_blocked1d_t(qw_sim *s, const void *in, void *out, int k) {
     return launch_blocked1d_k<R, M, KIND, false>(s, a);
 }
 
-// Sites per lane: larger M = larger tiles (better valid fraction) but more registers and code.
-template <typename R, int KIND> struct Blocked1dM { static constexpr int value = (KIND == COIN_HADAMARD) ? 16 : 8; };
-
+// Sites per lane: larger M = larger tiles (better valid fraction) but more registers and code.  The main launches use
+// M = 16 (Hadamard) / 8 (general coin) and depths that are multiples of M; a remainder of 4 .. 15 steps is mopped up by
+// one or two short launches with M = 8 / M = 4 tiles (one HBM round trip instead of 8 / 4 fused single steps).
 int blocked1d_granule(const qw_sim *s) {
     return s->coin_kind == COIN_HADAMARD ? 16 : 8;
 }
@@ -309,15 +310,22 @@ int blocked1d_max_k(const qw_sim *s) {
     return 8 * blocked1d_granule(s);
 }
 
-int launch_step_blocked1d(qw_sim *s, const void *in, void *out, int k) {
-    const int M = blocked1d_granule(s);
+template <typename R>
+static int launch_blocked1d_r(qw_sim *s, const void *in, void *out, int k) {
+    const bool had = s->coin_kind == COIN_HADAMARD;
+    const int M = (had && k % 16 == 0) ? 16 : (k % 8 == 0 ? 8 : 4);
     if (k <= 0 || k % M != 0 || 2 * k >= 32 * M) return fail(QW_EINVAL, "blocked step depth %d invalid for tile granule %d", k, M);
-    if (s->dtype == QW_C128) {
-        if (s->coin_kind == COIN_HADAMARD) return launch_blocked1d_t<double, 16, COIN_HADAMARD>(s, in, out, k);
-        return launch_blocked1d_t<double, 8, COIN_GENERAL>(s, in, out, k);
+    if (had) {
+        if (M == 16) return launch_blocked1d_t<R, 16, COIN_HADAMARD>(s, in, out, k);
+        if (M == 8) return launch_blocked1d_t<R, 8, COIN_HADAMARD>(s, in, out, k);
+        return launch_blocked1d_t<R, 4, COIN_HADAMARD>(s, in, out, k);
     }
-    if (s->coin_kind == COIN_HADAMARD) return launch_blocked1d_t<float, 16, COIN_HADAMARD>(s, in, out, k);
-    return launch_blocked1d_t<float, 8, COIN_GENERAL>(s, in, out, k);
+    if (M == 8) return launch_blocked1d_t<R, 8, COIN_GENERAL>(s, in, out, k);
+    return launch_blocked1d_t<R, 4, COIN_GENERAL>(s, in, out, k);
+}
+
+int launch_step_blocked1d(qw_sim *s, const void *in, void *out, int k) {
+    return s->dtype == QW_C128 ? launch_blocked1d_r<double>(s, in, out, k) : launch_blocked1d_r<float>(s, in, out, k);
 }
 
 }  // namespace qw

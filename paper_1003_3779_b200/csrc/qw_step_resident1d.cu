@@ -15,9 +15,9 @@
 
 namespace qw {
 
-// Launch shapes (sites per thread M, threads, CTAs per SM).  256-thread CTAs put exactly two warps on
-// every SM sub-partition and two CTAs on every SM (the second CTA hides the first one's barrier);
-// M = 9 lets 256 threads hold the 2049-site walks of BASELINE.json:configs[4].
+// Launch shapes (sites per thread M, threads, CTAs per SM) are chosen in launch_resident_t: two CTAs per SM (the
+// second one hides the first one's barrier) of up to 13 warps with M = 5 sites per thread for walks of up to 2080
+// sites (BASELINE.json:configs[4]: 2049), M = 6 up to 2304, one CTA of 512 threads x 8 sites up to 4096.
 constexpr int RES_MAX_SITES = 4096;
 
 template <typename R>
@@ -243,8 +243,10 @@ static int launch_resident_shape(qw_sim *s, const void *in, void *out, long long
 template <typename R, int KIND, bool PHASES>
 static int launch_resident_t(qw_sim *s, const void *in, void *out, long long n) {
     const long long N = s->g.en;
-    if (N <= 256 * 8) return launch_resident_shape<R, 8, KIND, PHASES, 256, 2>(s, in, out, n);
-    if (N <= 256 * 9) return launch_resident_shape<R, 9, KIND, PHASES, 256, 2>(s, in, out, n);
+    // measured on BASELINE.json:configs[4] (profiles/r01_blocked_resident.md, "launch shapes"): few sites per thread keep
+    // the M-step unrolled body inside the 32 KB instruction cache and make the light-cone test (per warp) finer
+    if (N <= 416 * 5) return launch_resident_shape<R, 5, KIND, PHASES, 416, 2>(s, in, out, n);
+    if (N <= 384 * 6) return launch_resident_shape<R, 6, KIND, PHASES, 384, 2>(s, in, out, n);
     return launch_resident_shape<R, 8, KIND, PHASES, 512, 1>(s, in, out, n);
 }
 
