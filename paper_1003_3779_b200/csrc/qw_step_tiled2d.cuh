@@ -51,6 +51,10 @@ struct Tiled2dArgs {
     // the scaled evaluation with coin_last = coin * scale^(K-1) (an exact power-of-two multiple)
     R coin_last[32];
     R ratio;                      // Grover-like: (d - g) / g
+    // light-cone DIAMOND (natural lattice: every step moves one site along one axis, so after t steps a delta start
+    // is confined to |m - m0| + |n - n0| <= t): tiles whose output sites all lie outside it are
+    // skipped (they are exact zeros in both buffers).  dia_r < 0: no diamond, every tile of the range is computed.
+    long long dia_m, dia_n, dia_r;
 };
 
 __host__ __device__ constexpr int t2d_mod(int a, int m) { return ((a % m) + m) % m; }
@@ -306,18 +310,33 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
         for (int c = 0; c < 4; ++c) t2d::tma_load_3d(stage + c * PLANE, &tmap, c0, c1, c * a.batch + (int)w, bar);
     };
 
+    // does tile t write a site that can be non-zero?  (uniform over the CTA)
+    auto active = [&](long long t) -> bool {
+        if (a.dia_r < 0) return true;
+        const long long r = t % per_walk;
+        const long long lo_m = (long long)(a.tile_m0 + (int)(r / a.tiles_n)) * TM, lo_n = (long long)(a.tile_n0 + (int)(r % a.tiles_n)) * TN;
+        const long long dm = a.dia_m < lo_m ? lo_m - a.dia_m : (a.dia_m > lo_m + TM - 1 ? a.dia_m - (lo_m + TM - 1) : 0);
+        const long long dn = a.dia_n < lo_n ? lo_n - a.dia_n : (a.dia_n > lo_n + TN - 1 ? a.dia_n - (lo_n + TN - 1) : 0);
+        return dm + dn <= a.dia_r;
+    };
+    auto next_active = [&](long long t) -> long long {
+        while (t < a.total_tiles && !active(t)) t += gridDim.x;
+        return t;
+    };
+
     if (tid == 0) {
         t2d::mbar_init(bar, 1);
         for (int i = 0; i < 2 * W; ++i) t2d::mbar_init(xbar + i, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    long long t = blockIdx.x;
+    long long t = next_active(blockIdx.x);
     if (tid == 0 && t < a.total_tiles) issue(t);
     const R *C = a.coin;                                           // kernel parameter = constant bank operands
     uint32_t phase = 0, xph = 0;
 
-    for (; t < a.total_tiles; t += gridDim.x) {
+    for (long long t_next; t < a.total_tiles; t = t_next) {
+        t_next = next_active(t + gridDim.x);
         const long long w = t / per_walk;
         const long long r = t - w * per_walk;
         const int tm = a.tile_m0 + (int)(r / a.tiles_n), tn = a.tile_n0 + (int)(r % a.tiles_n);
@@ -337,7 +356,7 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
             t2d::load_seg<RN>(stage + 3 * PLANE + off, p.c3[i]);
         }
         __syncthreads();
-        if (tid == 0 && t + gridDim.x < a.total_tiles) issue(t + gridDim.x);
+        if (tid == 0 && t_next < a.total_tiles) issue(t_next);
 
         // ---- K steps in registers
         bool wall_tile = false;

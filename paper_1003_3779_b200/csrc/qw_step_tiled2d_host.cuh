@@ -66,6 +66,14 @@ static int t2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     for (int i = 0; i < K - 1; ++i) pw *= scale;
     for (int i = 0; i < 32; ++i) a.coin_last[i] = (R)(s->h_coin[i] * pw);
     a.ratio = KIND == COIN_GROVER4 ? (R)((s->h_coin[0] - s->h_coin[2]) / s->h_coin[2]) : (R)0;
+    // diamond of the light cone after this launch; on a torus only while the square box has not wrapped
+    a.dia_r = -1; a.dia_m = s->centre[0]; a.dia_n = s->centre[1];
+    if (s->window_enabled && s->window_valid) {
+        const long long r = s->radius + K;
+        const bool wraps = g.boundary == QW_PERIODIC &&
+                           (a.dia_m - r < 0 || a.dia_m + r >= g.em || a.dia_n - r < 0 || a.dia_n + r >= g.en);
+        if (!wraps) a.dia_r = r;
+    }
     const size_t smem = tiled2d_smem_bytes<R>();
     const long long cap = (long long)s->sm_count;              // persistent: one CTA per SM
     const unsigned grid = (unsigned)(a.total_tiles < cap ? a.total_tiles : cap);
