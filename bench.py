@@ -54,17 +54,29 @@ def make_workload(name: str, walk_steps=None):
         return qi.k4(steps=walk_steps)
     if name == "k0":
         return qi.k0(steps=walk_steps or 100)
+    if name == "t1":
+        # context only: the largest row of the paper's Table 1 (1D segment of size 10000).  The paper
+        # does not state the number of iterations; iterations = size is SURVEY.md section 6's conjecture.
+        w = qi.k0(steps=walk_steps or 10000)
+        w.name, w.extents, w.delta_site = "T1", (10001,), (5000,)
+        return w
+    if name == "t2":
+        # context only: the largest row of the paper's Table 2 (2D DIAGONAL lattice, size 500), Fourier
+        # coin ("Fourier walker"); iterations = size is a conjecture, the precision is not stated
+        w = qi.k2(half=500, steps=walk_steps or 500)
+        w.name, w.lattice, w.coin = "T2", qi.DIAGONAL, qi.dft4(np.complex128)
+        return w
     raise SystemExit("unknown workload %r" % name)
 
 
 def workload_config(name, w, extra=None):
     cfg = {
         "workload": "%s: %dD %s lattice %s, batch %d, %s, coin %s, %d walk steps per bench step, outputs %s"
-                    % (w.name, w.dim, "periodic" if w.boundary == qi.PERIODIC else "open",
+                    % (w.name, w.dim, ("periodic" if w.boundary == qi.PERIODIC else "open") + (" DIAGONAL" if w.lattice == qi.DIAGONAL else ""),
                        "x".join(str(e) for e in w.extents), w.batch, np.dtype(w.dtype).name,
                        {0: "uniform", 1: "per-walk", 2: "per-site"}[w.coin_mode] + ("+site-phases" if w.phases is not None else ""),
                        w.steps, "+".join(w.outputs)),
-        "baseline_config": {"k0": 0, "k1": 1, "k1c64": 1, "k2": 2, "k3hxh": 3, "k3dft": 3, "k4": 4}[name],
+        "baseline_config": {"k0": 0, "k1": 1, "k1c64": 1, "k2": 2, "k3hxh": 3, "k3dft": 3, "k4": 4}.get(name),
         "sites": w.sites, "batch": w.batch, "walk_steps": w.steps,
         "l2": "working set (2 ping-pong state buffers) exceeds the 126 MB L2; no flush needed"
               if 2 * w.sites * w.batch * w.coin_dim * np.dtype(w.dtype).itemsize > 2 * 126e6 else
@@ -253,12 +265,15 @@ def oracle_sample(name: str, w, seconds_target: float = 12.0):
     elif name == "k4":
         sw = qi.k4(batch=64, half=1024, steps=32)
         desc = "64 of the 4096 walks x %d walk steps"
+    elif name in ("t1", "t2"):
+        sw = make_workload(name, 8)
+        desc = "the same lattice, %d walk steps"
     else:
         sw = qi.k0()
         desc = "the whole config (%d walk steps)"
     mode, coin = sw.general_coin_f64()
     psi = np.ascontiguousarray(sw.initial_state().astype(np.complex128))
-    kw = dict(boundary=sw.boundary, coin_mode=mode, batch=sw.batch)
+    kw = dict(boundary=sw.boundary, coin_mode=mode, batch=sw.batch, lattice=sw.lattice)
     # calibrate: one short call, then scale the step count to ~seconds_target
     t0 = time.perf_counter(); oracle.step(sw.extents, coin, psi, 1, **kw); t1 = time.perf_counter() - t0
     steps = int(max(1, min(4096, seconds_target / max(t1, 1e-6))))
@@ -540,7 +555,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="k1", choices=["k0", "k1", "k1c64", "k2", "k3hxh", "k3dft", "k4"])
+    ap.add_argument("--workload", default="k1", choices=["k0", "k1", "k1c64", "k2", "k3hxh", "k3dft", "k4", "t1", "t2"])
     ap.add_argument("--walk-steps", type=int, default=None, help="walk steps per bench step (default: the config's)")
     ap.add_argument("--schedule", default=None, choices=["auto", "generic", "fused", "blocked", "resident", "tiled"])
     ap.add_argument("--k", type=int, default=0)

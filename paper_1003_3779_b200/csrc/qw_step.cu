@@ -59,6 +59,19 @@ __device__ __forceinline__ unsigned philox4x32_10_word(unsigned c0, unsigned c1,
     return axis == 0 ? c0 : c1;
 }
 
+// Both words of one call: the states of the two links a site OWNS (axis 0 and axis 1).
+__device__ __forceinline__ void philox4x32_10_words01(unsigned c0, unsigned c1, unsigned c2, unsigned c3,
+                                                      unsigned k0, unsigned k1, unsigned &w0, unsigned &w1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const unsigned hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        c0 = hi1 ^ c1 ^ k0; c1 = lo1; c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    w0 = c0; w1 = c1;
+}
+
 // Is the link that component c of site (m,n) of walk w points along — it ends at (tm,tn) inside the lattice — broken
 // at step a.t?  The link is named by its OWNER (the end from which it points in the positive direction: dm > 0, or
 // dm = 0 and dn > 0) and its axis (0: along n / along (+1,+1); 1: along m / along (+1,-1)), so that both ends of a
@@ -100,6 +113,27 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
             for (int b = 0; b < CD; ++b) v[u][b] = cx_load<R>(a.in + b * a.plane_stride + idx);
         }
     }
+    // Random broken links on the natural lattice / in 1D: every site evaluates the ONE Philox call it owns (links to
+    // n+1 and to m+1); the link to n-1 is the left neighbour's: it comes through shared memory (the block's sites
+    // are consecutive along n), only the first site of a block recomputes it.  The link to m-1 belongs to another
+    // block's row and is recomputed.  2 -> 1 calls per site in 1D, 3 -> 2 in 2D.
+    constexpr bool SHARE = FAST && RBL && !DIAG;
+    __shared__ unsigned char link_n[SHARE ? U : 1][SHARE ? BS : 1];
+    unsigned own[U];
+    if constexpr (SHARE) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            own[u] = 0;
+            if (live[u]) {
+                const unsigned long long owner = (unsigned long long)(m * a.en + a.n_lo + n_base + (long long)u * BS);
+                unsigned w0, w1;
+                philox4x32_10_words01((unsigned)owner, (unsigned)(owner >> 32), a.t, (unsigned)w, a.rbl_key0, a.rbl_key1, w0, w1);
+                own[u] = ((unsigned long long)w0 < a.rbl_thr ? 1u : 0u) | ((unsigned long long)w1 < a.rbl_thr ? 2u : 0u);
+            }
+            link_n[u][threadIdx.x] = (unsigned char)(own[u] & 1u);
+        }
+        __syncthreads();
+    }
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         if (!live[u]) continue;
@@ -140,6 +174,18 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
             if constexpr (!FAST) {
                 if (a.broken && a.broken[(w * a.sites + x) * CD + c]) stay = true;
                 if (a.rbl && !stay && rbl_link_broken(a, w, m, n, tm, tn, dm, dn)) stay = true;
+            } else if constexpr (SHARE) {
+                if (!stay) {
+                    bool broken;
+                    if (dm == 0 && dn > 0) broken = (own[u] & 1u) != 0;                    // own link along n
+                    else if (dm > 0) broken = (own[u] & 2u) != 0;                          // own link along m
+                    else if (dm == 0) {                                                    // the left neighbour's link
+                        if (threadIdx.x > 0) broken = link_n[u][threadIdx.x - 1] != 0;
+                        else if (u > 0) broken = link_n[u > 0 ? u - 1 : 0][BS - 1] != 0;
+                        else broken = rbl_link_broken(a, w, m, n, tm, tn, dm, dn);         // first site of the block
+                    } else broken = rbl_link_broken(a, w, m, n, tm, tn, dm, dn);           // the upper row's link
+                    if (broken) stay = true;
+                }
             } else if constexpr (RBL) {
                 if (!stay && rbl_link_broken(a, w, m, n, tm, tn, dm, dn)) stay = true;
             }
