@@ -44,21 +44,62 @@ template <typename R> __device__ __forceinline__ cplx<R> cx_fma(R cre, R cim, cp
     acc.im = fma_rn(cim, z.re, acc.im);
     return acc;
 }
+// ---- complex64 on the packed FP32x2 pipe of sm_100 (FADD2 / FMUL2 / FFMA2: one instruction for re and im) ----------
+// IEEE round-to-nearest per component, no flush-to-zero: bit for bit the scalar result, half the issue slots.
+#ifndef QW_F32X2
+#define QW_F32X2 1
+#endif
+__device__ __forceinline__ unsigned long long f2_pack(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ cplx<float> f2_unpack(unsigned long long v) {
+    cplx<float> z;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(z.re), "=f"(z.im) : "l"(v));
+    return z;
+}
+__device__ __forceinline__ cplx<float> f2_add(cplx<float> a, cplx<float> b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(f2_pack(a.re, a.im)), "l"(f2_pack(b.re, b.im)));
+    return f2_unpack(r);
+}
+__device__ __forceinline__ cplx<float> f2_sub(cplx<float> a, cplx<float> b) {
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(f2_pack(a.re, a.im)), "l"(f2_pack(b.re, b.im)));
+    return f2_unpack(r);
+}
+__device__ __forceinline__ cplx<float> f2_mul(float sre, float sim, cplx<float> a) {        // (sre*a.re, sim*a.im)
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(f2_pack(sre, sim)), "l"(f2_pack(a.re, a.im)));
+    return f2_unpack(r);
+}
+__device__ __forceinline__ cplx<float> f2_fma(float sre, float sim, cplx<float> a, cplx<float> b) {   // (sre*a.re + b.re, sim*a.im + b.im)
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(f2_pack(sre, sim)), "l"(f2_pack(a.re, a.im)), "l"(f2_pack(b.re, b.im)));
+    return f2_unpack(r);
+}
+
 template <typename R> __device__ __forceinline__ cplx<R> cx_add(cplx<R> a, cplx<R> b) {
-    return cplx<R>{add_rn(a.re, b.re), add_rn(a.im, b.im)};
+    if constexpr (QW_F32X2 && sizeof(R) == 4) return f2_add(a, b);
+    else return cplx<R>{add_rn(a.re, b.re), add_rn(a.im, b.im)};
 }
 template <typename R> __device__ __forceinline__ cplx<R> cx_sub(cplx<R> a, cplx<R> b) {
-    return cplx<R>{sub_rn(a.re, b.re), sub_rn(a.im, b.im)};
+    if constexpr (QW_F32X2 && sizeof(R) == 4) return f2_sub(a, b);
+    else return cplx<R>{sub_rn(a.re, b.re), sub_rn(a.im, b.im)};
 }
 template <typename R> __device__ __forceinline__ cplx<R> cx_scale(R s, cplx<R> a) {
-    return cplx<R>{mul_rn(s, a.re), mul_rn(s, a.im)};
+    if constexpr (QW_F32X2 && sizeof(R) == 4) return f2_mul(s, s, a);
+    else return cplx<R>{mul_rn(s, a.re), mul_rn(s, a.im)};
 }
 // s * a + b,  s * a - b  with a real scale s
 template <typename R> __device__ __forceinline__ cplx<R> cx_fma_r(R s, cplx<R> a, cplx<R> b) {
-    return cplx<R>{fma_rn(s, a.re, b.re), fma_rn(s, a.im, b.im)};
+    if constexpr (QW_F32X2 && sizeof(R) == 4) return f2_fma(s, s, a, b);
+    else return cplx<R>{fma_rn(s, a.re, b.re), fma_rn(s, a.im, b.im)};
 }
 template <typename R> __device__ __forceinline__ cplx<R> cx_fms_r(R s, cplx<R> a, cplx<R> b) {
-    return cplx<R>{fma_rn(s, a.re, -b.re), fma_rn(s, a.im, -b.im)};
+    if constexpr (QW_F32X2 && sizeof(R) == 4) return f2_fma(s, s, a, cplx<R>{-b.re, -b.im});
+    else return cplx<R>{fma_rn(s, a.re, -b.re), fma_rn(s, a.im, -b.im)};
 }
 // i * a,  -i * a   (exact)
 template <typename R> __device__ __forceinline__ cplx<R> cx_muli(cplx<R> a)  { return cplx<R>{-a.im, a.re}; }
@@ -73,22 +114,16 @@ __device__ __forceinline__ void apply_coin(const R *__restrict__ C, cplx<R> (&v)
     if constexpr (KIND == COIN_HADAMARD && CD == 2) {
         // s*[[1,1],[1,-1]] as t = s*L; phi_R = s*R + t; phi_L = s*R - t: 2 mul + 4 fma per site
         const R s = C[0];
-        const R tre = mul_rn(s, v[1].re), tim = mul_rn(s, v[1].im);
-        const R are = v[0].re, aim = v[0].im;
-        v[0].re = fma_rn(s, are, tre);
-        v[0].im = fma_rn(s, aim, tim);
-        v[1].re = fma_rn(s, are, -tre);
-        v[1].im = fma_rn(s, aim, -tim);
+        const cplx<R> t = cx_scale(s, v[1]), r = v[0];
+        v[0] = cx_fma_r(s, r, t);
+        v[1] = cx_fms_r(s, r, t);
     } else if constexpr (KIND == COIN_GROVER4 && CD == 4) {
         // off-diagonal g, diagonal d (Grover: g = 1/2, d = -1/2): phi_a = g*sum + (d-g)*psi_a
         const R g = C[2], dg = sub_rn(C[0], C[2]);
         cplx<R> sum = cx_add(cx_add(v[0], v[1]), cx_add(v[2], v[3]));
         cplx<R> gs = cx_scale(g, sum);
 #pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            v[a].re = fma_rn(dg, v[a].re, gs.re);
-            v[a].im = fma_rn(dg, v[a].im, gs.im);
-        }
+        for (int a = 0; a < 4; ++a) v[a] = cx_fma_r(dg, v[a], gs);
     } else if constexpr (KIND == COIN_HXH4 && CD == 4) {
         // h * (H (x) H) with c = 2j+k.  The scale rides on the first butterfly (over k) as FMAs:
         // h*(x + y) = fma(h, x, h*y), then the butterfly over j: 2 mul + 4 fma + 4 add per real component.
@@ -138,10 +173,7 @@ __device__ __forceinline__ void apply_coin_bare(R r, cplx<R> (&v)[4]) {
     if constexpr (KIND == COIN_GROVER4) {
         const cplx<R> sum = cx_add(cx_add(v[0], v[1]), cx_add(v[2], v[3]));
 #pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            v[a].re = fma_rn(r, v[a].re, sum.re);
-            v[a].im = fma_rn(r, v[a].im, sum.im);
-        }
+        for (int a = 0; a < 4; ++a) v[a] = cx_fma_r(r, v[a], sum);
     } else if constexpr (KIND == COIN_HXH4) {
         const cplx<R> a0 = cx_add(v[0], v[1]), a1 = cx_sub(v[0], v[1]);
         const cplx<R> a2 = cx_add(v[2], v[3]), a3 = cx_sub(v[2], v[3]);
