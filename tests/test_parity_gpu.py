@@ -439,6 +439,34 @@ def test_light_cone_window_is_exact(qw, dev, wl):
 
 
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("coin", ["grover", "dft"])
+def test_light_cone_diamond_of_the_tiled_kernel(qw, oracle, dev, dtype, coin):
+    """The tiled 2D kernel skips every tile outside the cone's diamond |dm| + |dn| <= t (natural lattice).  Multi-tile
+    lattices, off-centre starts: (a) open, the diamond is cut by two walls and reflects; (b) torus, the diamond is used
+    until the cone's box wraps around, then switched off; (c) split stepping continues the same cone.  Window on ==
+    window off bit for bit, and parity with the oracle."""
+    c = {"grover": qi.grover4, "dft": qi.dft4}[coin](dtype)
+    dc = np.array([0.5, -0.5, -0.5, 0.5], dtype=dtype)
+    for boundary, ext, site, steps in ((qi.OPEN, (150, 210), (20, 170), 120), (qi.PERIODIC, (97, 130), (48, 65), 70)):
+        w = qi.Workload("dia", 2, ext, 1, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c, delta_site=site, delta_coin=dc)
+        on = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, window=True)
+        off = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
+        assert on[3]["sched"] == qw.QW_SCHED_TILED
+        assert np.array_equal(on[0], off[0]), (boundary, ext)
+        check_parity(w, on, oracle_run(oracle, w))
+        h = qw.create_for(w)
+        try:
+            qw.qw_set_schedule(h, qw.QW_SCHED_TILED, 0)
+            qw.load_state(h, w)
+            qw.qw_step(h, 13); qw.qw_step(h, steps - 13)
+            got = np.empty((1, w.sites, 4), dtype=w.dtype)
+            qw.qw_get_state(h, got)
+        finally:
+            qw.qw_destroy(h)
+        assert np.array_equal(got, off[0])
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 def test_translation_covariance_bit_exact(qw, dev, dtype):
     """P12: on a periodic lattice with a uniform coin, shifting psi0 by s sites shifts psi(t) by s."""
     w = qi.k1(sites=40000, steps=50, dtype=dtype)
