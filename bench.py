@@ -358,6 +358,10 @@ def run_gpu(args):
     qw.load()
 
     w = make_workload(args.workload, args.walk_steps)
+    if args.lattice == "diagonal":
+        if w.dim != 2:
+            raise SystemExit("--lattice diagonal needs a 2D workload")
+        w.lattice = qi.DIAGONAL                       # PAPER.md:106 Fig. 1c: the lattice of the paper's Tables 2-3
     real = np.float64 if w.dtype == np.complex128 else np.float32
     ebytes = np.dtype(w.dtype).itemsize
     site_updates_per_step = float(w.sites) * w.batch * w.steps
@@ -560,6 +564,7 @@ def main():
     ap.add_argument("--schedule", default=None, choices=["auto", "generic", "fused", "blocked", "resident", "tiled"])
     ap.add_argument("--k", type=int, default=0)
     ap.add_argument("--no-window", action="store_true")
+    ap.add_argument("--lattice", default=None, choices=["natural", "diagonal"], help="override the 2D lattice kind")
     ap.add_argument("--rbl", type=float, default=None, help="random broken links redrawn every step with this probability")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fused-leg", action="store_true")

@@ -388,8 +388,8 @@ int qw_step(qw_sim *s, int64_t n) {
                                      "lattice of >= %d sites or a natural 2D lattice of >= 32 x 32 sites",
                     32 * blocked1d_granule(s));
     if (sched == QW_SCHED_TILED && !tiled2d_eligible(s))
-        return fail(QW_EUNSUPPORTED, "the tiled schedule needs a uniform coin without phases or link mask on a natural 2D "
-                                     "lattice of >= 32 x 32 sites");
+        return fail(QW_EUNSUPPORTED, "the tiled schedule needs a uniform coin without phases or link mask on a 2D lattice of "
+                                     ">= 32 x 32 sites (diagonal lattice: a torus, or an open lattice with a delta start)");
     if (sched == QW_SCHED_TILED && s->sched_k != 0 && s->sched_k != 2 && s->sched_k != 4 && s->sched_k != 6 && s->sched_k != 8)
         return fail(QW_EINVAL, "the tiled schedule takes k = 2, 4, 6 or 8 (got %d)", s->sched_k);
     int64_t remaining = n;
@@ -400,6 +400,7 @@ int qw_step(qw_sim *s, int64_t n) {
         s->last_k = kmax;
         while (remaining >= 2) {
             const int kk = (int)(remaining >= kmax ? kmax : remaining / 2 * 2);
+            if (!tiled2d_diag_open_ok(s, kk)) break;       // the cone reaches a wall: the fused kernel (which has wall code) takes over
             const Box box = step_box(s, kk);
             int rc = launch_step_tiled2d(s, s->cur, 1 - s->cur, kk, box);
             if (rc) return rc;

@@ -156,6 +156,7 @@ int launch_ghost_refresh(qw_sim *s, int buf);     // periodic lattices: ghost ri
 // qw_step_tiled2d_*.cu : k in {2,4,6,8} steps per launch, persistent CTAs, tiles in REGISTERS, TMA prefetch
 // (uniform coin, 2D natural).  `box` = sites that can be non-zero after the launch (whole lattice if no window).
 bool tiled2d_eligible(const qw_sim *s);
+bool tiled2d_diag_open_ok(const qw_sim *s, int k);   // open diagonal lattice: k more steps cannot touch a wall
 int launch_step_tiled2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 int launch_tiled2d_f32(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 int launch_tiled2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);

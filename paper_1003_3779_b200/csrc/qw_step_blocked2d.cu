@@ -286,7 +286,29 @@ int launch_ghost_refresh(qw_sim *s, int buf) {
     return QW_OK;
 }
 
-bool tiled2d_eligible(const qw_sim *s) { return blocked2d_eligible(s); }
+// Natural lattice: as the shared-memory blocked kernel.  Diagonal lattice (no wall code): a torus, or an open lattice
+// with a known light cone — then tiled2d_diag_open_ok() must hold for every launch.
+bool tiled2d_eligible(const qw_sim *s) {
+    if (blocked2d_eligible(s)) return true;
+    const Geom &g = s->g;
+    const bool base = g.dim == 2 && g.lattice == QW_DIAGONAL && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
+                      !s->rbl && g.em >= 2 * QW_GHOST_2D && g.en >= 2 * QW_GHOST_2D && g.batch <= 16383 &&
+                      g.walk_stride * 4 * g.batch < (1LL << 40);
+    return base && (g.boundary == QW_PERIODIC || (s->window_enabled && s->window_valid));
+}
+
+// Open diagonal lattice: can k more steps be taken without any amplitude touching a wall?  The support after j steps
+// lies within Chebyshev distance radius + j of the start; a reflection at step j needs a wall site inside it.
+bool tiled2d_diag_open_ok(const qw_sim *s, int k) {
+    const Geom &g = s->g;
+    if (g.lattice != QW_DIAGONAL || g.boundary != QW_OPEN) return true;
+    if (!(s->window_enabled && s->window_valid)) return false;
+    long long d = s->centre[0];
+    if (g.em - 1 - s->centre[0] < d) d = g.em - 1 - s->centre[0];
+    if (s->centre[1] < d) d = s->centre[1];
+    if (g.en - 1 - s->centre[1] < d) d = g.en - 1 - s->centre[1];
+    return s->radius + k <= d;
+}
 
 // Register-tiled schedule: refresh the periodic halos, then dispatch on the dtype.
 int launch_step_tiled2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {

@@ -103,6 +103,10 @@ template <typename R> __device__ __forceinline__ cplx<R> shfl_down1(cplx<R> v) {
     return v;
 }
 
+template <typename R> __device__ __forceinline__ typename Cx<R>::T make_v(cplx<R> z) {
+    typename Cx<R>::T v; v.x = z.re; v.y = z.im; return v;
+}
+
 // A lane's row segment of RN consecutive sites: 16-byte vector accesses (shared or global memory).
 template <int RN> __device__ __forceinline__ void load_seg(const float2 *src, cplx<float> (&dst)[RN]) {
     static_assert(RN % 2 == 0, "complex64 segments are moved as float4");
@@ -272,16 +276,99 @@ struct Steps {
     }
 };
 
+// ---------------------------------------------------------------------------------------------------------------
+// DIAGONAL lattice (Fig. 1c, the lattice of the paper's Tables 2-3): component c = 2j+k moves BOTH
+// coordinates, (m + (-1)^j, n + (-1)^k).  Renaming at step s: the amplitude of logical site (i, j) lives in
+//     c0[(i-s) mod RM][(j-s) mod RN]   c1[(i-s) mod RM][(j+s) mod RN]
+//     c2[(i+s) mod RM][(j-s) mod RN]   c3[(i+s) mod RM][(j+s) mod RN]
+// Per step the edge COLUMN of every plane crosses a lane boundary (shuffles, all RM rows), then the edge ROW of every
+// plane (already holding the shuffled corner element) crosses a warp boundary through the exchange slots
+// xb[W][4][RN][32].  No wall code: the kernel is only launched where no amplitude can touch a wall (torus, or an
+// open lattice while the light cone stays inside: the dispatcher checks it per launch).
+template <typename R, int RM, int RN, int W, int KIND, int S, bool LAST>
+__device__ __forceinline__ void step_diag(Patch<R, RM, RN> &p, const R *C, const R *Clast, R ratio, typename Cx<R>::T *xb,
+                                          uint64_t *xbar, uint32_t &xph, int lane, int wid) {
+    typedef typename Cx<R>::T V;
+#pragma unroll
+    for (int i = 0; i < RM; ++i) {
+#pragma unroll
+        for (int j = 0; j < RN; ++j) {
+            const int im = t2d_mod(i - S, RM), ip = t2d_mod(i + S, RM), jm = t2d_mod(j - S, RN), jp = t2d_mod(j + S, RN);
+            cplx<R> v[4] = {p.c0[im][jm], p.c1[im][jp], p.c2[ip][jm], p.c3[ip][jp]};
+            if constexpr (KIND == COIN_GENERAL) apply_coin<R, 4, KIND>(C, v);
+            else if constexpr (LAST) apply_coin<R, 4, KIND>(Clast, v);
+            else apply_coin_bare<R, KIND>(ratio, v);
+            p.c0[im][jm] = v[0]; p.c1[im][jp] = v[1]; p.c2[ip][jm] = v[2]; p.c3[ip][jp] = v[3];
+        }
+    }
+    constexpr int QN = t2d_mod(RN - 1 - S, RN);   // column register of the planes moving n+1 (c0, c2) that leaves to the right
+    constexpr int PN = t2d_mod(S, RN);            // column register of the planes moving n-1 (c1, c3) that leaves to the left
+    constexpr int QM = t2d_mod(RM - 1 - S, RM);   // row register of the planes moving m+1 (c0, c1) that leaves downwards
+    constexpr int PM = t2d_mod(S, RM);            // row register of the planes moving m-1 (c2, c3) that leaves upwards
+    // ---- columns first (so that the corner element travels with its row afterwards)
+#pragma unroll
+    for (int r = 0; r < RM; ++r) {
+        p.c0[r][QN] = shfl_up1(p.c0[r][QN]);
+        p.c2[r][QN] = shfl_up1(p.c2[r][QN]);
+        p.c1[r][PN] = shfl_down1(p.c1[r][PN]);
+        p.c3[r][PN] = shfl_down1(p.c3[r][PN]);
+    }
+    // ---- rows through the exchange slots
+#pragma unroll
+    for (int j = 0; j < RN; ++j) {
+        xb[((wid * 4 + 0) * RN + j) * 32 + lane] = make_v<R>(p.c0[QM][j]);
+        xb[((wid * 4 + 1) * RN + j) * 32 + lane] = make_v<R>(p.c1[QM][j]);
+        xb[((wid * 4 + 2) * RN + j) * 32 + lane] = make_v<R>(p.c2[PM][j]);
+        xb[((wid * 4 + 3) * RN + j) * 32 + lane] = make_v<R>(p.c3[PM][j]);
+    }
+    constexpr bool NSYNC = T2dCfg<R>::NSYNC;
+    uint32_t par = 0;
+    if constexpr (NSYNC) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(xbar + wid);
+        par = (xph >> (S & 1)) & 1u;
+        xph ^= 1u << (S & 1);
+    } else {
+        __syncthreads();
+    }
+    if (wid > 0) {
+        if constexpr (NSYNC) mbar_wait(xbar + wid - 1, par);
+#pragma unroll
+        for (int j = 0; j < RN; ++j) {
+            p.c0[QM][j] = cx_load<R>(xb + (((wid - 1) * 4 + 0) * RN + j) * 32 + lane);
+            p.c1[QM][j] = cx_load<R>(xb + (((wid - 1) * 4 + 1) * RN + j) * 32 + lane);
+        }
+    }
+    if (wid < W - 1) {
+        if constexpr (NSYNC) mbar_wait(xbar + wid + 1, par);
+#pragma unroll
+        for (int j = 0; j < RN; ++j) {
+            p.c2[PM][j] = cx_load<R>(xb + (((wid + 1) * 4 + 2) * RN + j) * 32 + lane);
+            p.c3[PM][j] = cx_load<R>(xb + (((wid + 1) * 4 + 3) * RN + j) * 32 + lane);
+        }
+    }
+}
+
+template <typename R, int RM, int RN, int W, int KIND, int S, int K>
+struct StepsDiag {
+    static __device__ __forceinline__ void run(Patch<R, RM, RN> &p, const R *C, const R *Clast, R ratio, typename Cx<R>::T *xch,
+                                               uint64_t *xbar, uint32_t &xph, int lane, int wid) {
+        step_diag<R, RM, RN, W, KIND, S, S + 1 == K>(p, C, Clast, ratio, xch + (S & 1) * (W * 4 * RN * 32), xbar + (S & 1) * W, xph,
+                                                     lane, wid);
+        if constexpr (S + 1 < K) StepsDiag<R, RM, RN, W, KIND, S + 1, K>::run(p, C, Clast, ratio, xch, xbar, xph, lane, wid);
+    }
+};
+
 }  // namespace t2d
 
-template <typename R> constexpr size_t tiled2d_smem_bytes() {
+template <typename R, bool DIAG = false> constexpr size_t tiled2d_smem_bytes() {
     typedef T2dCfg<R> G;
     return (size_t)4 * (G::W * G::RM) * (32 * G::RN) * sizeof(typename Cx<R>::T)      // TMA stage
-         + (size_t)2 * G::W * 2 * G::RN * 32 * sizeof(typename Cx<R>::T)              // exchange slots
+         + (size_t)2 * G::W * (DIAG ? 4 : 2) * G::RN * 32 * sizeof(typename Cx<R>::T) // exchange slots
          + (size_t)(2 * G::W + 2) * 8;                                                // mbarriers
 }
 
-template <typename R, int KIND, bool OPEN, int K>
+template <typename R, int KIND, bool OPEN, int K, bool DIAG = false>
 __global__ void __launch_bounds__(T2dCfg<R>::W * 32, 1)
 step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<R> a) {
     typedef typename Cx<R>::T V;
@@ -294,11 +381,12 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
     static_assert(sizeof(V) == 16 || K % 2 == 0, "complex64 tiles need an even halo (16-byte aligned TMA box origin)");
     static_assert(RN * sizeof(V) % 16 == 0, "a lane's row segment must be a whole number of 16-byte vectors");
     static_assert(K % RN == 0, "the halo must be a whole number of lane segments");
+    static_assert(!(DIAG && OPEN), "the diagonal-lattice steps have no wall code (see step_diag)");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     V *stage = reinterpret_cast<V *>(smem_raw);                    // stage[c][row][col]
-    V *xch = stage + 4 * PLANE;                                    // xch[parity][warp][2][RN][32]
-    uint64_t *bar = reinterpret_cast<uint64_t *>(xch + 2 * W * 2 * RN * 32);   // "stage is full"
+    V *xch = stage + 4 * PLANE;                                    // xch[parity][warp][2 (diagonal: 4)][RN][32]
+    uint64_t *bar = reinterpret_cast<uint64_t *>(xch + 2 * W * (DIAG ? 4 : 2) * RN * 32);   // "stage is full"
     uint64_t *xbar = bar + 2;                                      // xbar[parity][warp]: "slot of the warp is full"
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -374,7 +462,10 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
             wl.jl = (jl >= 0 && jl < RN) ? (int)jl : -1;
             wl.jr = (jr >= 0 && jr < RN) ? (int)jr : -1;
         }
-        t2d::Steps<R, RM, RN, W, KIND, OPEN, 0, K>::run(p, C, a.coin_last, a.ratio, xch, xbar, xph, lane, wid, wall_tile, wl);
+        if constexpr (DIAG)
+            t2d::StepsDiag<R, RM, RN, W, KIND, 0, K>::run(p, C, a.coin_last, a.ratio, xch, xbar, xph, lane, wid);
+        else
+            t2d::Steps<R, RM, RN, W, KIND, OPEN, 0, K>::run(p, C, a.coin_last, a.ratio, xch, xbar, xph, lane, wid, wall_tile, wl);
 
         // ---- store the valid interior straight from registers: psi_c(i, j) after K steps sits at
         //      c0[i][(j-K) mod RN], c1[(i-K) mod RM][j], c2[(i+K) mod RM][j], c3[i][(j+K) mod RN]
@@ -392,10 +483,17 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
                 cplx<R> z0[RN], z1[RN], z2[RN], z3[RN];
 #pragma unroll
                 for (int j = 0; j < RN; ++j) {
-                    z0[j] = p.c0[i][t2d_mod(j - K, RN)];
-                    z1[j] = p.c1[t2d_mod(i - K, RM)][j];
-                    z2[j] = p.c2[t2d_mod(i + K, RM)][j];
-                    z3[j] = p.c3[i][t2d_mod(j + K, RN)];
+                    if constexpr (DIAG) {
+                        z0[j] = p.c0[t2d_mod(i - K, RM)][t2d_mod(j - K, RN)];
+                        z1[j] = p.c1[t2d_mod(i - K, RM)][t2d_mod(j + K, RN)];
+                        z2[j] = p.c2[t2d_mod(i + K, RM)][t2d_mod(j - K, RN)];
+                        z3[j] = p.c3[t2d_mod(i + K, RM)][t2d_mod(j + K, RN)];
+                    } else {
+                        z0[j] = p.c0[i][t2d_mod(j - K, RN)];
+                        z1[j] = p.c1[t2d_mod(i - K, RM)][j];
+                        z2[j] = p.c2[t2d_mod(i + K, RM)][j];
+                        z3[j] = p.c3[i][t2d_mod(j + K, RN)];
+                    }
                 }
                 t2d::store_seg<RN>(row + 0 * a.plane_stride, z0);
                 t2d::store_seg<RN>(row + 1 * a.plane_stride, z1);
@@ -405,10 +503,17 @@ step_tiled2d_kernel(const __grid_constant__ CUtensorMap tmap, const Tiled2dArgs<
 #pragma unroll
                 for (int j = 0; j < RN; ++j) {
                     if (gn0 + j < a.en) {
-                        cx_store<R>(row + 0 * a.plane_stride + j, p.c0[i][t2d_mod(j - K, RN)]);
-                        cx_store<R>(row + 1 * a.plane_stride + j, p.c1[t2d_mod(i - K, RM)][j]);
-                        cx_store<R>(row + 2 * a.plane_stride + j, p.c2[t2d_mod(i + K, RM)][j]);
-                        cx_store<R>(row + 3 * a.plane_stride + j, p.c3[i][t2d_mod(j + K, RN)]);
+                        if constexpr (DIAG) {
+                            cx_store<R>(row + 0 * a.plane_stride + j, p.c0[t2d_mod(i - K, RM)][t2d_mod(j - K, RN)]);
+                            cx_store<R>(row + 1 * a.plane_stride + j, p.c1[t2d_mod(i - K, RM)][t2d_mod(j + K, RN)]);
+                            cx_store<R>(row + 2 * a.plane_stride + j, p.c2[t2d_mod(i + K, RM)][t2d_mod(j - K, RN)]);
+                            cx_store<R>(row + 3 * a.plane_stride + j, p.c3[t2d_mod(i + K, RM)][t2d_mod(j + K, RN)]);
+                        } else {
+                            cx_store<R>(row + 0 * a.plane_stride + j, p.c0[i][t2d_mod(j - K, RN)]);
+                            cx_store<R>(row + 1 * a.plane_stride + j, p.c1[t2d_mod(i - K, RM)][j]);
+                            cx_store<R>(row + 2 * a.plane_stride + j, p.c2[t2d_mod(i + K, RM)][j]);
+                            cx_store<R>(row + 3 * a.plane_stride + j, p.c3[i][t2d_mod(j + K, RN)]);
+                        }
                     }
                 }
             }

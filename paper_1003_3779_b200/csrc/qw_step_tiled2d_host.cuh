@@ -68,13 +68,14 @@ static int t2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     a.ratio = KIND == COIN_GROVER4 ? (R)((s->h_coin[0] - s->h_coin[2]) / s->h_coin[2]) : (R)0;
     // diamond of the light cone after this launch; on a torus only while the square box has not wrapped
     a.dia_r = -1; a.dia_m = s->centre[0]; a.dia_n = s->centre[1];
-    if (s->window_enabled && s->window_valid) {
+    const bool diag = g.lattice == QW_DIAGONAL;      // both coordinates move: the cone is the square, no diamond
+    if (!diag && s->window_enabled && s->window_valid) {
         const long long r = s->radius + K;
         const bool wraps = g.boundary == QW_PERIODIC &&
                            (a.dia_m - r < 0 || a.dia_m + r >= g.em || a.dia_n - r < 0 || a.dia_n + r >= g.en);
         if (!wraps) a.dia_r = r;
     }
-    const size_t smem = tiled2d_smem_bytes<R>();
+    const size_t smem = diag ? tiled2d_smem_bytes<R, true>() : tiled2d_smem_bytes<R, false>();
     const long long cap = (long long)s->sm_count;              // persistent: one CTA per SM
     const unsigned grid = (unsigned)(a.total_tiles < cap ? a.total_tiles : cap);
     const CUtensorMap &tm = *reinterpret_cast<const CUtensorMap *>(s->tmap_t[in_buf]);
@@ -83,7 +84,9 @@ static int t2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
         kernel<<<grid, G::W * 32, smem, s->stream>>>(tm, a);
         return QW_OK;
     };
-    int rc = g.boundary == QW_OPEN ? go(step_tiled2d_kernel<R, KIND, true, K>) : go(step_tiled2d_kernel<R, KIND, false, K>);
+    // diagonal lattice: no wall code in the kernel; the dispatcher only comes here when no amplitude can touch a wall
+    int rc = diag ? go(step_tiled2d_kernel<R, KIND, false, K, true>)
+                  : (g.boundary == QW_OPEN ? go(step_tiled2d_kernel<R, KIND, true, K>) : go(step_tiled2d_kernel<R, KIND, false, K>));
     if (rc) return rc;
     QW_LAUNCH_CHECK(s, "step_tiled2d_kernel");
     return QW_OK;

@@ -439,6 +439,59 @@ def test_light_cone_window_is_exact(qw, dev, wl):
 
 
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("coin", ["grover", "hxh", "dft", "random"])
+def test_tiled_2d_diagonal_lattice_is_bit_identical_to_single_steps(qw, oracle, dev, dtype, coin):
+    """The lattice of the paper's Tables 2-3 (Fig. 1c) in the register-tiled kernel: every plane crosses
+    lanes AND warps each step (corner elements travel with their row).  Torus, random state: several tiles with ragged
+    tails, fewer and more tiles than SMs, every depth K; tiled == fused bit for bit, and parity with the oracle."""
+    rng = np.random.default_rng(14)
+    for extents, steps, k, batch in (((97, 130), 21, 0, 1), ((64, 64), 9, 2, 3), ((33, 200), 17, 4, 1),
+                                     ((150, 41), 26, 6, 1), ((500, 700), 16, 8, 1), ((35, 32), 8, 8, 2)):
+        c = {"grover": qi.grover4, "hxh": qi.hadamard_x_hadamard, "dft": qi.dft4}[coin](dtype) if coin != "random" \
+            else qi.random_unitary(rng, 4).astype(dtype)
+        sites = extents[0] * extents[1]
+        w = qi.Workload("dgt2d", 2, extents, batch, qi.PERIODIC, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
+                        state=qi.random_state(33, batch, sites, 4, dtype, normalise_per_walk=True), lattice=qi.DIAGONAL)
+        a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k)
+        assert b[3]["sched"] == qw.QW_SCHED_TILED
+        assert np.array_equal(a[0], b[0]), (extents, steps, k)
+        if sites < 20000:
+            check_parity(w, b, oracle_run(oracle, w))
+    assert gpu_run(qw, w)[3]["sched"] == qw.QW_SCHED_TILED                     # the AUTO schedule on a diagonal torus
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+def test_tiled_2d_diagonal_lattice_delta_start(qw, oracle, dev, dtype, boundary):
+    """Delta start on the diagonal lattice (the paper's Table 2 workload in small): the tiled kernel has no wall code, so
+    on an open lattice the dispatcher hands over to the fused kernel when the light cone reaches a wall, and on a torus
+    the window is dropped when the cone wraps.  Off-centre start, more steps than the distance to the nearest wall."""
+    c = qi.dft4(dtype)
+    dc = np.array([0.5, -0.5, -0.5, 0.5], dtype=dtype)
+    w = qi.Workload("dgd", 2, (140, 170), 1, boundary, np.dtype(dtype), 90, qi.COIN_UNIFORM, c, delta_site=(40, 100),
+                    delta_coin=dc, lattice=qi.DIAGONAL)
+    ref = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
+    for window in (True, False) if boundary == qi.PERIODIC else (True,):
+        t = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, window=window)
+        assert np.array_equal(ref[0], t[0]), window
+    auto = gpu_run(qw, w)
+    assert np.array_equal(ref[0], auto[0])
+    check_parity(w, auto, oracle_run(oracle, w))
+    if boundary == qi.OPEN:                       # launch count: the first 40 - 8 steps at least were blocked
+        assert auto[3]["launches"] < ref[3]["launches"] - 20
+        h = qw.create_for(w)
+        try:
+            qw.qw_set_schedule(h, qw.QW_SCHED_TILED, 0)
+            qw.qw_set_state(h, w.initial_state())                               # general state on an open diagonal lattice
+            with pytest.raises(qw.QwError) as ei:
+                qw.qw_step(h, 8)
+            assert ei.value.code == qw.QW_EUNSUPPORTED
+        finally:
+            qw.qw_destroy(h)
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 @pytest.mark.parametrize("coin", ["grover", "dft"])
 def test_light_cone_diamond_of_the_tiled_kernel(qw, oracle, dev, dtype, coin):
     """The tiled 2D kernel skips every tile outside the cone's diamond |dm| + |dn| <= t (natural lattice).  Multi-tile
