@@ -421,7 +421,11 @@ int qw_step(qw_sim *s, int64_t n) {
     }
     if (sched == QW_SCHED_BLOCKED) {
         const int M = blocked1d_granule(s);
-        int kmax = s->sched_k > 0 ? s->sched_k : 48;     // measured optimum on B200 (profiles/r01_blocked1d.md)
+        int kmax = s->sched_k > 0 ? s->sched_k : 48;     // measured optimum on B200 (profiles/r01_blocked1d_v2.md)
+        // a lattice with fewer tiles than resident warps is launch bound (a launch costs ~50 us whatever k, mostly
+        // instruction fetch): take the deepest launches instead
+        if (s->sched_k == 0 && s->g.batch * ((s->g.en + (32 * M - 96) - 1) / (32 * M - 96)) < 8LL * s->sm_count)
+            kmax = blocked1d_max_k(s);
         if (kmax > blocked1d_max_k(s)) kmax = blocked1d_max_k(s);
         kmax = kmax / M * M;
         if (kmax < M) kmax = M;

@@ -45,7 +45,7 @@ template <typename R> __device__ __forceinline__ cplx<R> shfl_down1(cplx<R> v) {
     return v;
 }
 
-// One walk step with s = U (mod M).  x0 = unwrapped coordinate of this lane's logical site 0.
+// One walk step with s = U (mod M).
 //
 // Deferred scale (KIND == COIN_HADAMARD with M = 16; the short M = 8 / M = 4 tiles that mop up a remainder of 4 .. 15
 // steps use the scaled evaluation of the fused kernel, bit for bit): the coin s*[[1,1],[1,-1]] is linear in s, so M consecutive steps equal
@@ -57,7 +57,7 @@ template <typename R> __device__ __forceinline__ cplx<R> shfl_down1(cplx<R> v) {
 // <= 4 ulp per step (SURVEY.md 8(c) P13 "otherwise <= 4 ulp t").
 template <typename R, int M, int KIND, bool OPEN, int U>
 __device__ __forceinline__ void blocked1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
-                                               bool wall_warp, long long x0, long long n_sites) {
+                                               int lane, int lo_lane, int hi_lane) {
 #pragma unroll
     for (int i = 0; i < M; ++i) {
         const int q = (i - U + M) % M, p = (i + U) % M;
@@ -79,34 +79,26 @@ __device__ __forceinline__ void blocked1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M
     constexpr int QS = (M - 1 - U + M) % M;     // holds phi_R of logical M-1, becomes R' of logical 0
     constexpr int PS = U % M;                   // holds phi_L of logical 0,   becomes L' of logical M-1
     if constexpr (OPEN) {
-        // reflecting walls (PAPER.md:94-101 with RBL = 0): R'[0] = phi_L[0], L'[N-1] = phi_R[N-1]
-        if (wall_warp) {
-            cplx<R> fixR = {0, 0}, fixL = {0, 0};
-#pragma unroll
-            for (int i = 0; i < M; ++i) {
-                if (x0 + i == 0) fixR = Lp[(i + U) % M];
-                if (x0 + i == n_sites - 1) fixL = Rp[(i - U + M) % M];
-            }
-            Rp[QS] = shfl_up1(Rp[QS]);
-            Lp[PS] = shfl_down1(Lp[PS]);
-#pragma unroll
-            for (int i = 0; i < M; ++i) {
-                if (x0 + i == 0) Rp[(i - U - 1 + 2 * M) % M] = fixR;
-                if (x0 + i == n_sites - 1) Lp[(i + U + 1) % M] = fixL;
-            }
-            return;
-        }
+        // reflecting walls (PAPER.md:94-101 with RBL = 0): R'[0] = phi_L[0], L'[N-1] = phi_R[N-1].  The tiles are laid out
+        // so that site 0 is always logical site 0 of lane lo_lane (first tile of a walk) and site N-1 logical site M-1 of
+        // lane hi_lane (last tile, which ends exactly at the wall): the reflected value replaces what the shuffle brings.
+        const cplx<R> outR = Rp[QS], outL = Lp[PS];
+        Rp[QS] = shfl_up1(outR);
+        Lp[PS] = shfl_down1(outL);
+        if (lane == lo_lane) Rp[QS] = outL;
+        if (lane == hi_lane) Lp[PS] = outR;
+    } else {
+        Rp[QS] = shfl_up1(Rp[QS]);
+        Lp[PS] = shfl_down1(Lp[PS]);
     }
-    Rp[QS] = shfl_up1(Rp[QS]);
-    Lp[PS] = shfl_down1(Lp[PS]);
 }
 
 template <typename R, int M, int KIND, bool OPEN, int U>
 struct Blocked1dUnroll {
-    static __device__ __forceinline__ void run(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C, bool wall_warp,
-                                               long long x0, long long n_sites) {
-        blocked1d_step<R, M, KIND, OPEN, U>(Rp, Lp, C, wall_warp, x0, n_sites);
-        if constexpr (U + 1 < M) Blocked1dUnroll<R, M, KIND, OPEN, U + 1>::run(Rp, Lp, C, wall_warp, x0, n_sites);
+    static __device__ __forceinline__ void run(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C, int lane, int lo_lane,
+                                               int hi_lane) {
+        blocked1d_step<R, M, KIND, OPEN, U>(Rp, Lp, C, lane, lo_lane, hi_lane);
+        if constexpr (U + 1 < M) Blocked1dUnroll<R, M, KIND, OPEN, U + 1>::run(Rp, Lp, C, lane, lo_lane, hi_lane);
     }
 };
 
@@ -156,6 +148,12 @@ step_blocked1d_kernel(const Blocked1dArgs<R> a) {
         const unsigned q = (unsigned)tid / (unsigned)a.tiles_per_walk;
         w = q; t = (long long)((unsigned)tid - q * (unsigned)a.tiles_per_walk);
     };
+    // unwrapped coordinate of element 0 of tile t of a walk.  Open lattice: the LAST tile is shifted so that it ends exactly
+    // at the wall (its outputs are the last `valid` sites; the tile before it stores only what lies in front of them)
+    auto tile_start = [&](long long t) -> long long {
+        if (OPEN && t == a.tiles_per_walk - 1) return N - a.valid - a.k;
+        return t * a.valid - a.k;
+    };
     // element i*32 + lane of a tile sits at stage_pos(lane) + i * STEP_I of a staging plane (M divides 32)
     constexpr int STEP_I = (32 / M) * (M + 1);
     const int pos_lane = stage_pos<M>(lane);
@@ -164,7 +162,7 @@ step_blocked1d_kernel(const Blocked1dArgs<R> a) {
     auto prefetch = [&](long long tid) {
         long long w, t;
         split(tid, w, t);
-        const long long start = t * a.valid - a.k;
+        const long long start = tile_start(t);
         const V *inw = a.in + w * a.walk_stride;
         if (start >= 0 && start + 32 * M <= N) {             // interior tile: no wrap, no wall -> immediate offsets only
             const V *p0 = inw + start + lane, *p1 = p0 + a.plane_stride;
@@ -199,7 +197,7 @@ step_blocked1d_kernel(const Blocked1dArgs<R> a) {
     for (; tile_id < a.total_tiles; tile_id += stride) {
         long long w, t;
         split(tile_id, w, t);
-        const long long start = t * a.valid - a.k;     // unwrapped coordinate of tile element 0
+        const long long start = tile_start(t);         // unwrapped coordinate of tile element 0
         V *outw = a.out + w * a.walk_stride;
 
         // ---- padded shared -> lane-contiguous registers
@@ -216,16 +214,22 @@ step_blocked1d_kernel(const Blocked1dArgs<R> a) {
         if (tile_id + stride < a.total_tiles) prefetch(tile_id + stride);
 
         // ---- k steps in registers
-        const long long x0 = start + (long long)lane * M;
-        bool wall_warp = false;
-        if (OPEN) wall_warp = (start <= 0) || (start + 32 * M >= N);
+        int lo_lane = -1, hi_lane = -1;                // lanes that own site 0 (as logical site 0) / site N-1 (as logical M-1)
+        if (OPEN) {
+            if (t == 0) lo_lane = a.k / M;
+            if (t == a.tiles_per_walk - 1) hi_lane = 31 - a.k / M;
+        }
         for (int s = 0; s < a.k; s += M)
-            Blocked1dUnroll<R, M, KIND, OPEN, 0>::run(Rp, Lp, C, wall_warp, x0, N);
+            Blocked1dUnroll<R, M, KIND, OPEN, 0>::run(Rp, Lp, C, lane, lo_lane, hi_lane);
 
         // ---- store the valid middle: registers -> padded shared -> coalesced global
-        const bool whole = (t + 1) * a.valid <= N;          // every valid output site of the tile is inside the lattice
+        // sites this tile stores: [start + k, x_end).  Ring: the last tile is cut at N.  Open lattice: the tile before the
+        // (shifted) last one is cut where the last one begins.
+        const long long x_end_all = OPEN ? N - a.valid : N;
+        const long long x_end = (OPEN && t == a.tiles_per_walk - 1) ? N : x_end_all;
+        const bool whole = start + a.k + a.valid <= x_end;  // every valid output site of the tile is stored
         const int lk = lane - a.k;                          // element e = i*32 + lane is valid iff 0 <= e - k < valid
-        V *o0 = outw + (t * a.valid + lk);
+        V *o0 = outw + (start + a.k + lk);
 #pragma unroll
         for (int plane = 0; plane < 2; ++plane) {
 #pragma unroll
@@ -243,7 +247,7 @@ step_blocked1d_kernel(const Blocked1dArgs<R> a) {
             } else {
 #pragma unroll 4
                 for (int i = 0; i < M; ++i)
-                    if ((unsigned)(lk + i * 32) < (unsigned)a.valid && t * a.valid + lk + i * 32 < N)
+                    if ((unsigned)(lk + i * 32) < (unsigned)a.valid && start + a.k + lk + i * 32 < x_end)
                         op[i * 32] = st_out[pos_lane + i * STEP_I];
             }
             __syncwarp();
