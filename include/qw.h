@@ -60,17 +60,21 @@ enum { QW_PERIODIC = 0, QW_OPEN = 1 };
 enum { QW_NATURAL = 0, QW_DIAGONAL = 1 };
 enum { QW_COIN_UNIFORM = 0, QW_COIN_PER_WALK = 1, QW_COIN_PER_SITE = 2 };
 
-/* Step schedules (qw_set_schedule).  All schedules compute bit-identical states. */
+/* Step schedules (qw_set_schedule). */
 enum {
     QW_SCHED_AUTO = 0,     /* library picks: resident if a walk fits one CTA, else blocked (1D) / tiled
-                              (2D) / fused                                                              */
+                              (2D) / fused.  All schedules give bit-identical states except the blocked 1D
+                              schedule with the Hadamard coin, whose scale is applied once per 16 steps
+                              (<= 4 ulp per step from the others)                    */
     QW_SCHED_GENERIC = 1,  /* one launch per step, one thread per site, every feature (reference kernel) */
     QW_SCHED_FUSED = 2,    /* one launch per step, vectorised fused coin+shift (HBM-bound)              */
     QW_SCHED_BLOCKED = 3,  /* temporally blocked: k steps per HBM round trip (1D: register tiles per warp;
                               2D: shared-memory tiles loaded by TMA)                                    */
     QW_SCHED_RESIDENT = 4, /* one CTA per walk, state on the SM for all n steps                         */
     QW_SCHED_TILED = 5     /* 2D temporally blocked, tiles held in REGISTERS by persistent CTAs with TMA
-                              prefetch; k in {2, 4, 6, 8}; honours the light-cone window                */
+                              prefetch; k in {2, 4, 6, 8}; honours the light-cone window.  Natural lattice:
+                              any boundary.  Diagonal lattice: torus, or open lattice after
+                              qw_set_state_delta (the fused kernel takes over when the cone reaches a wall) */
 };
 
 /* qw_get_info keys */

@@ -13,6 +13,9 @@
 //           index is a compile-time constant; k must be a multiple of M.
 // No block-level synchronisation and no shared-memory traffic inside the k steps; shared memory
 // is only the staging area that turns coalesced global accesses into lane-contiguous registers.
+// Warps are persistent and prefetch their next tile with cp.async while the current one is advanced;
+// the Hadamard coin runs with a deferred scale; open lattices align their first / last tile with the
+// walls; a remainder of 4 .. 15 steps uses short M = 8 / M = 4 tiles (all explained where they occur).
 // HBM bytes per site-step: coin_dim*sizeof(complex) * (32M/valid + 1) / k  instead of 2*coin_dim*sizeof(complex).
 #include "qw_coin.cuh"
 
