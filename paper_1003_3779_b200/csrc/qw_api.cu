@@ -421,7 +421,9 @@ int qw_step(qw_sim *s, int64_t n) {
     }
     if (sched == QW_SCHED_BLOCKED) {
         const int M = blocked1d_granule(s);
-        int kmax = s->sched_k > 0 ? s->sched_k : 48;     // measured optimum on B200 (profiles/r01_blocked1d_v2.md)
+        // measured optima on B200 (profiles/r01_blocked1d_v2.md): Hadamard (512-site tiles, 4 FP instr per site-step) k = 48;
+        // general coin (256-site tiles, 16 FP instr per site-step: the halo recomputation costs more than the HBM trips) k = 16
+        int kmax = s->sched_k > 0 ? s->sched_k : (M == 16 ? 48 : 16);
         // a lattice with fewer tiles than resident warps is launch bound (a launch costs ~50 us whatever k, mostly
         // instruction fetch): take the deepest launches instead
         if (s->sched_k == 0 && s->g.batch * ((s->g.en + (32 * M - 96) - 1) / (32 * M - 96)) < 8LL * s->sm_count)
