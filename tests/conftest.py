@@ -10,7 +10,16 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
-    config.addinivalue_line("markers", "slow: long-running full-size parity case")
+    config.addinivalue_line("markers", "slow: long-running full-size parity case (skipped unless QW_RUN_SLOW=1)")
+
+
+def pytest_collection_modifyitems(config, items):
+    if os.environ.get("QW_RUN_SLOW") == "1":
+        return
+    skip = pytest.mark.skip(reason="slow full-size case: set QW_RUN_SLOW=1")
+    for item in items:
+        if "slow" in item.keywords:
+            item.add_marker(skip)
 
 
 @pytest.fixture(scope="session")

@@ -97,28 +97,49 @@ def test_k1_full_size_sampled_light_cones(qw, oracle, dev, dtype):
 
 
 # ------------------------------------------------------------------ K3: torus 8192^2, complex64
-@pytest.mark.parametrize("coin,steps,nsamples", [("hxh", 96, 6), ("dft", 96, 6), ("dft", 500, 1)])
+def oracle_patch_2d(oracle, init, E, coin, centre, steps, pad, stage=100):
+    """Amplitudes of the (2*pad+1)^2 patch around `centre` after `steps` steps, from the oracle alone.
+
+    The patch depends only on the initial state within `steps` + pad sites of it (eq. 18 :210).  The
+    oracle evolves that window with open ends; what the (wrong) ends emit travels inwards one site per step, so after
+    every `stage` steps the outer `stage` sites are dropped and the rest is still exact.  This is scheduling of calls
+    to oracle.step, not a change of its arithmetic."""
+    cm, cn = centre
+    half = steps + pad
+    im = np.arange(cm - half, cm + half + 1) % E
+    inn = np.arange(cn - half, cn + half + 1) % E
+    win = np.ascontiguousarray(init[np.ix_(im, inn)].astype(np.complex128))
+    done = 0
+    while done < steps:
+        d = min(stage, steps - done)
+        side = win.shape[0]
+        flat = np.ascontiguousarray(win.reshape(1, side * side, 4))
+        oracle.step((side, side), coin, flat, d, boundary=qi.OPEN)
+        win = np.ascontiguousarray(flat.reshape(side, side, 4)[d:side - d, d:side - d])
+        done += d
+    assert win.shape[0] == 2 * pad + 1
+    return win, (im[half - pad:half + pad + 1], inn[half - pad:half + pad + 1])
+
+
+@pytest.mark.parametrize("coin,steps,nsamples", [("hxh", 96, 6), ("dft", 96, 6), ("hxh", 500, 4), ("dft", 500, 4)])
 def test_k3_full_size_sampled_light_cones(qw, oracle, dev, coin, steps, nsamples):
+    """BASELINE.json:configs[3] at its full size and (500) its full step count, both coins: >= 4 light-cone patches
+    each (the torus seam in both directions, a tile corner of the 64 x 64 register tiles, the lattice centre)."""
     w = qi.k3(coin=coin, steps=steps)
     E = w.extents[0]
     final, mom, P, info = run_full(qw, w)
+    assert info["sched"] == qw.QW_SCHED_TILED                 # the configuration bench.py times
     init = w.state[0].reshape(E, E, 4)
     fin = final[0].reshape(E, E, 4)
     rng = np.random.default_rng(2)
     centres = [(0, 0), (E - 1, 17), (E // 2, E - 1), (4095, 4096)][:nsamples] + \
         [tuple(int(v) for v in rng.integers(0, E, 2)) for _ in range(max(0, nsamples - 4))]
     pad = 2
-    half = steps + pad
     c128 = w.coin.astype(np.complex128)
     worst = 0.0
-    for (cm, cn) in centres:
-        im = np.arange(cm - half, cm + half + 1) % E
-        inn = np.arange(cn - half, cn + half + 1) % E
-        win = np.ascontiguousarray(init[np.ix_(im, inn)].astype(np.complex128)).reshape(1, -1, 4)
-        side = 2 * half + 1
-        oracle.step((side, side), c128, win, steps, boundary=qi.OPEN)
-        want = win.reshape(side, side, 4)[half - pad:half + pad + 1, half - pad:half + pad + 1]
-        got = fin[np.ix_(im[half - pad:half + pad + 1], inn[half - pad:half + pad + 1])].astype(np.complex128)
+    for centre in centres:
+        want, (rm, rn) = oracle_patch_2d(oracle, init, E, c128, centre, steps, pad)
+        got = fin[np.ix_(rm, rn)].astype(np.complex128)
         worst = max(worst, float(np.max(np.abs(got - want))))
     assert worst <= 2e-5, worst
     assert abs(mom[0, 0] - 1) <= 1e-4
@@ -127,25 +148,67 @@ def test_k3_full_size_sampled_light_cones(qw, oracle, dev, coin, steps, nsamples
 
 
 # ------------------------------------------------------------------ K2: open 4097^2 Grover walk
-def test_k2_full_lattice_300_steps_against_the_whole_light_cone(qw, oracle, dev):
-    """Full 4097^2 lattice, 300 steps: the oracle evolves the whole (2*300+3)^2 support."""
-    steps = 300
+def oracle_delta_cone_2d(oracle, w_of_half, steps, stage=128):
+    """The oracle's state of a delta-start walk after `steps` steps on the lattice of half-width steps + 1.
+
+    A delta start is supported within t sites of its origin after t steps (eq. 18 :210) and everything
+    outside is exactly zero, so the oracle may run the first t steps on any open lattice whose half-width exceeds t:
+    the state is embedded in a larger lattice of zeros every `stage` steps.  Scheduling of oracle calls only."""
+    done, psi, half = 0, None, 0
+    while done < steps:
+        d = min(stage, steps - done)
+        nh = done + d + 1
+        wo = w_of_half(nh)
+        side = 2 * nh + 1
+        if psi is None:
+            big = wo.initial_state().reshape(side, side, 4)
+        else:
+            big = np.zeros((side, side, 4), dtype=np.complex128)
+            o = nh - half
+            big[o:o + 2 * half + 1, o:o + 2 * half + 1] = psi
+        flat = np.ascontiguousarray(big.reshape(1, side * side, 4))
+        oracle.step(wo.extents, wo.coin, flat, d, boundary=qi.OPEN)
+        psi, half, done = flat.reshape(side, side, 4), nh, done + d
+    return psi, half
+
+
+def k2_against_the_whole_cone(qw, oracle, steps):
     w = qi.k2(steps=steps)
     final, mom, P, info = run_full(qw, w)
-    half = steps + 1
+    assert info["sched"] == qw.QW_SCHED_TILED                 # the configuration bench.py times (diamond tile skip on)
+    psi, half = oracle_delta_cone_2d(oracle, lambda h: qi.k2(half=h, steps=1), steps)
     side = 2 * half + 1
-    wo = qi.k2(half=half, steps=steps)
-    psi = wo.initial_state()
-    oracle.step(wo.extents, wo.coin, psi, steps, boundary=qi.OPEN)
     fin = final[0].reshape(4097, 4097, 4)
     c = 2048
-    got = fin[c - half:c + half + 1, c - half:c + half + 1]
-    assert np.max(np.abs(got - psi.reshape(side, side, 4))) <= 1e-12
+    lo, hi = max(0, c - half), min(4097, c + half + 1)        # 2048 steps: the cone's pad row lies outside the lattice
+    o = lo - (c - half)
+    want = psi[o:o + hi - lo, o:o + hi - lo]
+    assert not psi[:o].any() and not psi[:, :o].any()         # ... and holds zeros only
+    got = fin[lo:hi, lo:hi]
+    err = float(np.max(np.abs(got - want)))
+    assert err <= 1e-12, err
     outside = fin.copy()
-    outside[c - half:c + half + 1, c - half:c + half + 1] = 0
+    outside[lo:hi, lo:hi] = 0
     assert not outside.any()                                   # exact zeros outside the cone
-    Po = oracle.probabilities(wo.extents, psi)[0].reshape(side, side)
-    assert np.max(np.abs(P[0].reshape(4097, 4097)[c - half:c + half + 1, c - half:c + half + 1] - Po)) <= 1e-12
+    Po = oracle.probabilities((side, side), np.ascontiguousarray(psi.reshape(1, side * side, 4)))[0].reshape(side, side)
+    perr = float(np.max(np.abs(P[0].reshape(4097, 4097)[lo:hi, lo:hi] - Po[o:o + hi - lo, o:o + hi - lo])))
+    assert perr <= 1e-12, perr
+    return err, perr, info
+
+
+def test_k2_full_lattice_1024_steps_against_the_whole_light_cone(qw, oracle, dev):
+    """Full 4097^2 lattice, 1024 of the config's 2048 steps, element by element over the WHOLE cone (2051^2 sites):
+    the diamond tile-skip logic of the tiled kernel runs 1024 steps under an element-wise check."""
+    k2_against_the_whole_cone(qw, oracle, 1024)
+
+
+@pytest.mark.slow
+def test_k2_full_config_2048_steps_against_the_whole_light_cone(qw, oracle, dev):
+    """BASELINE.json:configs[2] exactly: 2048 steps, every amplitude and probability of the 4097^2 lattice against the
+    oracle (about 15 min of oracle time: run with QW_RUN_SLOW=1; the builder's log line is kept in profiles/)."""
+    err, perr, info = k2_against_the_whole_cone(qw, oracle, 2048)
+    print("K2 full config, 2048 steps, element-wise over 4097^2 sites: max|d amp| = %.3e, max|d P| = %.3e, launches = %d"
+          % (err, perr, info["launches"]))
 
 
 def test_k2_full_config_invariants(qw, oracle, dev):

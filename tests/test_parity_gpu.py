@@ -111,12 +111,33 @@ def test_k1_ring_twins(qw, oracle, dev, dtype, sites, steps):
     check_parity(w, gpu_run(qw, w), oracle_run(oracle, w))
 
 
+@pytest.mark.parametrize("sites,coin,k", [((1 << 20) + 3, "hadamard", 48), ((1 << 20) + 3, "su2", 16)])
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+def test_k1_prime_twin_every_site(qw, oracle, dev, dtype, sites, coin, k):
+    """SURVEY.md 8(d) K1' at its stated size: a ring of 2^20 + 3 sites x 200 steps, EVERY site against the oracle,
+    through the temporally blocked schedule at an explicit depth and as AUTO picks it.  2^20 sites are more tiles
+    than the grid has warps, so the persistent multi-tile loop with its prefetch runs under an element-wise check
+    (Hadamard: 512-site tiles, deferred scale; SU(2): 256-site tiles, M = 8)."""
+    w = qi.k1(sites=sites, steps=200, dtype=dtype)
+    if coin == "su2":
+        w.coin = qi.su2(0.7, 1.1, 2.3).astype(dtype)
+    ora = oracle_run(oracle, w)
+    for schedule, kk in ((qw.QW_SCHED_BLOCKED, k), (qw.QW_SCHED_AUTO, 0)):
+        gpu = gpu_run(qw, w, schedule=schedule, k=kk)
+        assert gpu[3]["sched"] == qw.QW_SCHED_BLOCKED and gpu[3]["launches"] <= 200 // 8
+        check_parity(w, gpu, ora)
+
+
 @pytest.mark.parametrize("half,steps", [(64, 64), (40, 100)])
 def test_k2_grover_twins(qw, oracle, dev, half, steps):
     w = qi.k2(half=half, steps=steps)                                # steps > half: the wall reflects
     gpu = gpu_run(qw, w)
     check_parity(w, gpu, oracle_run(oracle, w))
     if steps <= half:
+        # GPU-side mirror symmetry (m -> -m, m <-> n), NOT an oracle gate.  The bound is 1e-15 rather than bit equality
+        # because the Grover evaluation g*((v0+v1)+(v2+v3)) + (d-g)*v_a (qw_coin.cuh, DESIGN.md section 2 "Arithmetic
+        # choice") adds the four components in a fixed order: mirroring the lattice permutes v0..v3 (c0 <-> c3, c1 <-> c2),
+        # so the mirrored site rounds its sum differently by <= 1 ulp per step.  Probabilities here are <= 0.25.
         P = gpu[1][0].reshape(w.extents)
         assert np.max(np.abs(P - P[::-1, :])) < 1e-15 and np.max(np.abs(P - P.T)) < 1e-15
 
@@ -266,7 +287,7 @@ def test_blocked_1d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, d
         else:
             assert np.array_equal(a[0], b[0]), (sites, steps, k)
             assert np.array_equal(a[0], auto[0])
-    check_parity(w, b, oracle_run(oracle, w))
+        check_parity(w, b, oracle_run(oracle, w))                     # every configuration, not only the last
 
 
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
