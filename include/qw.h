@@ -68,7 +68,8 @@ enum {
                               (<= 4 ulp per step from the others)                    */
     QW_SCHED_GENERIC = 1,  /* one launch per step, one thread per site, every feature (reference kernel) */
     QW_SCHED_FUSED = 2,    /* one launch per step, vectorised fused coin+shift (HBM-bound)              */
-    QW_SCHED_BLOCKED = 3,  /* temporally blocked: k steps per HBM round trip (1D: register tiles per warp;
+    QW_SCHED_BLOCKED = 3,  /* temporally blocked: k steps per HBM round trip (1D: register tiles per warp —
+                              on a ring chained through the stream of L amplitudes, no halo recomputation;
                               2D: shared-memory tiles loaded by TMA)                                    */
     QW_SCHED_RESIDENT = 4, /* one CTA per walk, state on the SM for all n steps                         */
     QW_SCHED_TILED = 5     /* 2D temporally blocked, tiles held in REGISTERS by persistent CTAs with TMA
@@ -85,6 +86,17 @@ enum {
     QW_INFO_LAST_K = 3,         /* temporal block depth of the last qw_step (1 if not blocked)           */
     QW_INFO_STATE_BYTES = 4,    /* bytes of one device state buffer (there are two)                      */
     QW_INFO_WINDOW = 5          /* 1 if the light-cone window is active                                  */
+};
+
+/* qw_set_option keys */
+enum {
+    QW_OPT_MAX_CTAS = 0,        /* cap on the grid of the persistent (blocked 1D) kernels; 0 = one grid
+                                   that fills every SM (default).  For sharing a GPU and for tests that want
+                                   long per-warp tile chains on small lattices; results do not depend on it */
+    QW_OPT_BLOCKED1D_KERNEL = 1 /* which temporally blocked 1D kernel QW_SCHED_BLOCKED uses on a ring: 0 = the
+                                   cheaper one (default), 1 = warp tiles with recomputed halos, 2 = chained
+                                   tiles (no halo work; rings with a uniform coin, else falls back to 1).
+                                   Both execute the same arithmetic per site: bit-identical results          */
 };
 
 /* Create a walk on a dim-dimensional lattice (dim = 1 or 2) with `extents[d] >= 1` sites per
@@ -169,6 +181,9 @@ int qw_set_schedule(qw_sim *s, int schedule, int k);
 /* Enable (1, default) / disable (0) the light-cone window: after qw_set_state_delta only sites
  * within t+1 of the start are updated at step t.  Exact: skipped sites are 0. */
 int qw_set_window(qw_sim *s, int enable);
+
+/* Tuning knobs that never change results (QW_OPT_*).  QW_EINVAL for an unknown key or a bad value. */
+int qw_set_option(qw_sim *s, int key, int64_t value);
 
 int qw_get_info(const qw_sim *s, int what, int64_t *out);
 

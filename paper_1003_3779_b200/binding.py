@@ -22,13 +22,14 @@ QW_NATURAL, QW_DIAGONAL = 0, 1
 QW_COIN_UNIFORM, QW_COIN_PER_WALK, QW_COIN_PER_SITE = 0, 1, 2
 QW_SCHED_AUTO, QW_SCHED_GENERIC, QW_SCHED_FUSED, QW_SCHED_BLOCKED, QW_SCHED_RESIDENT, QW_SCHED_TILED = 0, 1, 2, 3, 4, 5
 QW_INFO_LAUNCHES, QW_INFO_TIME, QW_INFO_LAST_SCHEDULE, QW_INFO_LAST_K, QW_INFO_STATE_BYTES, QW_INFO_WINDOW = range(6)
+QW_OPT_MAX_CTAS, QW_OPT_BLOCKED1D_KERNEL = 0, 1
 
 # every symbol include/qw.h declares (tests/test_abi.py checks the header against this list)
 SYMBOLS = (
     "qw_create", "qw_create_batch", "qw_destroy", "qw_set_stream", "qw_set_lattice", "qw_set_coin",
     "qw_set_site_phases", "qw_set_broken_links", "qw_set_random_broken_links", "qw_set_state", "qw_set_state_delta", "qw_get_state",
     "qw_step", "qw_step_inverse", "qw_probabilities", "qw_moments", "qw_set_schedule", "qw_set_window",
-    "qw_get_info", "qw_synchronize", "qw_last_error",
+    "qw_set_option", "qw_get_info", "qw_synchronize", "qw_last_error",
 )
 
 
@@ -72,6 +73,7 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
         "qw_moments": [vp, vp],
         "qw_set_schedule": [vp, ci, ci],
         "qw_set_window": [vp, ci],
+        "qw_set_option": [vp, ci, i64],
         "qw_get_info": [vp, ci, i64p],
         "qw_synchronize": [vp],
     }
@@ -190,6 +192,10 @@ def qw_set_schedule(h, schedule, k=0) -> None:
 
 def qw_set_window(h, enable) -> None:
     _check(load().qw_set_window(h, int(enable)))
+
+
+def qw_set_option(h, key, value) -> None:
+    _check(load().qw_set_option(h, int(key), int(value)))
 
 
 def qw_get_info(h, what) -> int:

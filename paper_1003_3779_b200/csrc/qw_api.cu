@@ -204,6 +204,10 @@ int qw_set_lattice(qw_sim *s, int lattice) {
     if (!s) return fail(QW_EINVAL, "handle is NULL");
     if (lattice != QW_NATURAL && lattice != QW_DIAGONAL) return fail(QW_EINVAL, "unknown lattice kind %d", lattice);
     if (s->g.dim == 1 && lattice == QW_DIAGONAL) return fail(QW_EINVAL, "the diagonal lattice is 2D only");
+    // The light-cone bookkeeping (`radius`: Chebyshev distance, and the L1 diamond the tiled kernel derives from it) counts
+    // one axis move per step of the NATURAL lattice; steps taken on the other lattice spread differently, so a change of
+    // lattice in mid-walk drops the window (exactness first; qw_set_state_delta re-arms it).
+    if (lattice != s->g.lattice && s->has_state && s->t != 0) s->window_valid = false;
     s->g.lattice = lattice;
     return QW_OK;
 }
@@ -421,8 +425,9 @@ int qw_step(qw_sim *s, int64_t n) {
     }
     if (sched == QW_SCHED_BLOCKED) {
         const int M = blocked1d_granule(s);
-        // measured optima on B200 (profiles/r01_blocked1d_v2.md): Hadamard (512-site tiles, 4 FP instr per site-step) k = 48;
-        // general coin (256-site tiles, 16 FP instr per site-step: the halo recomputation costs more than the HBM trips) k = 16
+        // Halo kernel (qw_step_blocked1d.cu), measured optima on B200 (profiles/r01_blocked1d_v2.md): Hadamard (512-site
+        // tiles, 4 FP instr per site-step) k = 48; general coin (256-site tiles, 16 FP instr per site-step: the halo
+        // recomputation costs more than the HBM trips) k = 16
         int kmax = s->sched_k > 0 ? s->sched_k : (M == 16 ? 48 : 16);
         // a lattice with fewer tiles than resident warps is launch bound (a launch costs ~50 us whatever k, mostly
         // instruction fetch): take the deepest launches instead
@@ -431,12 +436,28 @@ int qw_step(qw_sim *s, int64_t n) {
         if (kmax > blocked1d_max_k(s)) kmax = blocked1d_max_k(s);
         kmax = kmax / M * M;
         if (kmax < M) kmax = M;
-        s->last_k = kmax;
+        // Chain kernel (qw_step_chain1d.cu; rings): no halo recomputation, one starter tile per chain instead.  Depth:
+        // the user's k, else the deepest its FIFO holds.  It is taken whenever it advances a step with fewer tile
+        // computations per warp than the halo kernel (always, on lattices of many tiles per warp).
+        int kchain = s->sched_k > 0 ? s->sched_k : chain1d_max_k(s);
+        if (kchain > chain1d_max_k(s)) kchain = chain1d_max_k(s);
+        kchain = kchain / M * M;
+        bool chain = kchain >= M && chain1d_eligible(s, kchain);
+        if (chain && s->blocked1d_kernel == 0) chain = chain1d_cost(s, kchain) / kchain < blocked1d_cost(s, kmax) / kmax;
+        if (s->blocked1d_kernel == 1) chain = false;
+        s->last_k = chain ? kchain : kmax;
         // multiples of M with the big tiles, then a remainder of 4 .. 15 steps with short 8- / 4-step launches (small
         // tiles, the fused kernel's arithmetic), then at most 3 fused single steps
         while (remaining >= 4) {
-            const int kk = remaining >= M ? (int)(remaining >= kmax ? kmax : remaining / M * M) : (remaining >= 8 ? 8 : 4);
-            int rc = launch_step_blocked1d(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), kk);
+            int rc;
+            int kk;
+            if (chain && remaining >= M) {
+                kk = (int)(remaining >= kchain ? kchain : remaining / M * M);
+                rc = launch_step_chain1d(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), kk);
+            } else {
+                kk = remaining >= M ? (int)(remaining >= kmax ? kmax : remaining / M * M) : (remaining >= 8 ? 8 : 4);
+                rc = launch_step_blocked1d(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), kk);
+            }
             if (rc) return rc;
             s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;
         }
@@ -508,6 +529,23 @@ int qw_set_schedule(qw_sim *s, int schedule, int k) {
     if (schedule < QW_SCHED_AUTO || schedule > QW_SCHED_TILED) return fail(QW_EINVAL, "unknown schedule %d", schedule);
     if (k < 0) return fail(QW_EINVAL, "k must be >= 0");
     s->sched = schedule; s->sched_k = k;
+    return QW_OK;
+}
+
+int qw_set_option(qw_sim *s, int key, int64_t value) {
+    clear_error();
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    switch (key) {
+        case QW_OPT_MAX_CTAS:
+            if (value < 0 || value > 0x7fffffff) return fail(QW_EINVAL, "QW_OPT_MAX_CTAS must be >= 0");
+            s->max_ctas = (int)value;
+            break;
+        case QW_OPT_BLOCKED1D_KERNEL:
+            if (value < 0 || value > 2) return fail(QW_EINVAL, "QW_OPT_BLOCKED1D_KERNEL must be 0 (auto), 1 (halo tiles) or 2 (chained tiles)");
+            s->blocked1d_kernel = (int)value;
+            break;
+        default: return fail(QW_EINVAL, "unknown option key %d", key);
+    }
     return QW_OK;
 }
 

@@ -82,6 +82,8 @@ struct qw_sim {
     long long radius;        // support of psi(t) is within `radius` of `centre` (Chebyshev)
 
     // schedule
+    int max_ctas;            // QW_OPT_MAX_CTAS: cap on the grid of the persistent kernels (0 = all SMs)
+    int blocked1d_kernel;    // QW_OPT_BLOCKED1D_KERNEL: 0 = cheaper of the two, 1 = halo tiles, 2 = chained tiles (rings)
     int sched, sched_k;
     int last_sched, last_k;
     long long launches;
@@ -141,6 +143,14 @@ bool blocked1d_eligible(const qw_sim *s);
 int blocked1d_granule(const qw_sim *s);
 int blocked1d_max_k(const qw_sim *s);
 int launch_step_blocked1d(qw_sim *s, const void *in, void *out, int k);
+
+// qw_step_chain1d.cu : k steps per launch on a ring, tiles chained through the stream of L amplitudes (no halo work)
+bool chain1d_eligible(const qw_sim *s, int k);
+int chain1d_granule(const qw_sim *s);
+int chain1d_max_k(const qw_sim *s);
+double chain1d_cost(qw_sim *s, int k);               // tile computations per warp of one launch
+int launch_step_chain1d(qw_sim *s, const void *in, void *out, int k);
+double blocked1d_cost(const qw_sim *s, int k);       // same for the halo kernel
 
 // qw_step_resident1d.cu : one CTA per walk, all n steps on the SM (1D walks of <= 4096 sites)
 bool resident1d_eligible(const qw_sim *s);

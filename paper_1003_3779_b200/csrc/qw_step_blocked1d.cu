@@ -262,7 +262,8 @@ template <typename R, int M, int KIND, bool OPEN>
 static int launch_blocked1d_k(qw_sim *s, const Blocked1dArgs<R> &a) {
     auto kern = step_blocked1d_kernel<R, M, KIND, OPEN>;
     constexpr size_t smem = blocked1d_smem_bytes<R, M>();
-    static int ctas_per_sm = 0;      // per instantiation; the device is fixed for the life of the process' handles
+    static int ctas_per_sm_dev[64];  // per instantiation AND per device: the function attribute is a per-device setting
+    int &ctas_per_sm = ctas_per_sm_dev[s->device & 63];
     if (ctas_per_sm == 0) {
         QW_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int n = 0;
@@ -272,7 +273,8 @@ static int launch_blocked1d_k(qw_sim *s, const Blocked1dArgs<R> &a) {
     }
     if (a.total_tiles > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
     long long blocks = (a.total_tiles + BLK1D_WARPS - 1) / BLK1D_WARPS;
-    const long long resident = (long long)s->sm_count * ctas_per_sm;
+    long long resident = (long long)s->sm_count * ctas_per_sm;
+    if (s->max_ctas > 0 && resident > s->max_ctas) resident = s->max_ctas;
     if (blocks > resident) blocks = resident;
     kern<<<(unsigned)blocks, BLK1D_WARPS * 32, smem, s->stream>>>(a);
     QW_LAUNCH_CHECK(s, "step_blocked1d_kernel");
@@ -310,6 +312,18 @@ bool blocked1d_eligible(const qw_sim *s) {
     const Geom &g = s->g;
     return g.dim == 1 && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken && !s->rbl &&
            g.en >= 32LL * blocked1d_granule(s);
+}
+
+// Tile computations per warp of one k-step launch (the halo kernel recomputes 2k of every 32*M sites).
+double blocked1d_cost(const qw_sim *s, int k) {
+    const int M = (s->coin_kind == COIN_HADAMARD && k % 16 == 0) ? 16 : (k % 8 == 0 ? 8 : 4);
+    const long long valid = 32LL * M - 2LL * k;
+    if (valid <= 0) return 1e300;
+    const long long tiles = (s->g.en + valid - 1) / valid * s->g.batch;
+    long long ctas = (long long)s->sm_count * (s->dtype == QW_C128 ? 2 : 4);
+    if (s->max_ctas > 0 && ctas > s->max_ctas) ctas = s->max_ctas;
+    const long long warps = ctas * BLK1D_WARPS;
+    return (double)((tiles + warps - 1) / warps);
 }
 
 int blocked1d_max_k(const qw_sim *s) {

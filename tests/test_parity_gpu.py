@@ -30,11 +30,13 @@ def real_dtype(w):
     return np.float64 if w.dtype == np.complex128 else np.float32
 
 
-def gpu_run(qw, w, steps=None, schedule=None, k=0, window=True, inverse=0, broken=None, get_state=True):
+def gpu_run(qw, w, steps=None, schedule=None, k=0, window=True, inverse=0, broken=None, get_state=True, options=None):
     """Run workload w on the GPU; returns (amps AoS in w.dtype, P, moments, info)."""
     steps = w.steps if steps is None else steps
     h = qw.create_for(w)
     try:
+        for key, value in (options or {}).items():
+            qw.qw_set_option(h, key, value)
         if broken is not None:
             qw.qw_set_broken_links(h, broken)
         if schedule is not None:
@@ -288,6 +290,37 @@ def test_blocked_1d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, d
             assert np.array_equal(a[0], b[0]), (sites, steps, k)
             assert np.array_equal(a[0], auto[0])
         check_parity(w, b, oracle_run(oracle, w))                     # every configuration, not only the last
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("coin", ["hadamard", "su2"])
+def test_chained_blocked_1d_kernel(qw, oracle, dev, dtype, coin):
+    """The chained ring kernel (qw_step_chain1d.cu: tiles in the frame moving with the R plane, the L outflow of a tile
+    fed to its left neighbour through a FIFO, one redundant starter tile per chain) against the halo kernel (bit for
+    bit: same arithmetic per site), the fused single steps and the oracle.  QW_OPT_MAX_CTAS shrinks the persistent
+    grid so that small rings give chains of many tiles; sizes: ragged last chain / last tile, a batch, the minimal
+    ring of two tiles, chains of one tile, every depth, several launches with a remainder."""
+    rng = np.random.default_rng(23)
+    M = 16 if coin == "hadamard" else 8
+    cases = ((20000, 112, 48, 1, 1), (3001, 64, 16, 3, 2), (70001, 131, 0, 1, 0), (64 * M, 64, 64, 2, 1),
+             (100003, 200, 64, 1, 3), (9973, 40, 32, 2, 1))
+    for sites, steps, k, batch, max_ctas in cases:
+        c = qi.hadamard(dtype) if coin == "hadamard" else qi.su2(*rng.uniform(0, 2 * np.pi, 3)).astype(dtype)
+        w = qi.Workload("chain", 1, (sites,), batch, qi.PERIODIC, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
+                        state=qi.random_state(11, batch, sites, 2, dtype, normalise_per_walk=True))
+        opt = {qw.QW_OPT_MAX_CTAS: max_ctas}
+        chain = gpu_run(qw, w, schedule=qw.QW_SCHED_BLOCKED, k=k, options={**opt, qw.QW_OPT_BLOCKED1D_KERNEL: 2})
+        halo = gpu_run(qw, w, schedule=qw.QW_SCHED_BLOCKED, k=k if k <= 48 else 48, options={**opt, qw.QW_OPT_BLOCKED1D_KERNEL: 1})
+        assert chain[3]["sched"] == qw.QW_SCHED_BLOCKED
+        assert np.array_equal(chain[0], halo[0]), (sites, steps, k, batch)
+        fused = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        if coin == "hadamard":      # deferred scale: <= 4 ulp per step from the scaled single steps (DESIGN.md section 2)
+            eps = np.finfo(np.float64 if dtype == np.complex128 else np.float32).eps
+            bound = 4 * eps * steps * float(np.max(np.abs(fused[0])))
+            assert np.max(np.abs(fused[0].astype(np.complex128) - chain[0].astype(np.complex128))) <= bound
+        else:
+            assert np.array_equal(chain[0], fused[0]), (sites, steps, k, batch)
+        check_parity(w, chain, oracle_run(oracle, w))
 
 
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
