@@ -370,6 +370,9 @@ def run_gpu(args):
     h = qw.create_for(w)
     if args.schedule is not None:
         qw.qw_set_schedule(h, {"auto": 0, "generic": 1, "fused": 2, "blocked": 3, "resident": 4, "tiled": 5}[args.schedule], args.k)
+    for kv in args.opt:
+        key, value = kv.split("=")
+        qw.qw_set_option(h, int(key), int(value))
     if args.no_window:
         qw.qw_set_window(h, 0)
     if args.rbl is not None:
@@ -566,6 +569,8 @@ def main():
     ap.add_argument("--no-window", action="store_true")
     ap.add_argument("--lattice", default=None, choices=["natural", "diagonal"], help="override the 2D lattice kind")
     ap.add_argument("--rbl", type=float, default=None, help="random broken links redrawn every step with this probability")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="qw_set_option(key, value) by number, e.g. --opt 1=1 forces the halo kernel of the blocked 1D schedule")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fused-leg", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -41,18 +41,54 @@ struct Chain1dArgs {
     R scale_m;               // deferred-scale Hadamard: s^M, applied once per M steps
 };
 
-template <typename R> __device__ __forceinline__ cplx<R> chain_shfl_down1(cplx<R> v) {
-    v.re = __shfl_down_sync(0xffffffffu, v.re, 1);
-    v.im = __shfl_down_sync(0xffffffffu, v.im, 1);
+// ---- exchange by warp shuffles (complex64) -------------------------------------------------------------------------
+template <typename R> __device__ __forceinline__ cplx<R> chain_shfl_from(cplx<R> v, int src) {
+    v.re = __shfl_sync(0xffffffffu, v.re, src);
+    v.im = __shfl_sync(0xffffffffu, v.im, src);
     return v;
 }
+// if (take) { a = p[0]; b = p[1]; } as predicated shared-memory loads INTO the registers that hold a and b
+__device__ __forceinline__ void chain_fifo_load_in_place(const float2 *p, unsigned take, cplx<float> &a, cplx<float> &b) {
+    const unsigned addr = (unsigned)__cvta_generic_to_shared(p);
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
+                 "@p ld.shared.v4.f32 {%0, %1, %2, %3}, [%5];\n\t}"
+                 : "+f"(a.re), "+f"(a.im), "+f"(b.re), "+f"(b.im) : "r"(take), "r"(addr) : "memory");
+}
+__device__ __forceinline__ void chain_fifo_load_in_place(const double2 *p, unsigned take, cplx<double> &a, cplx<double> &b) {
+    const unsigned addr = (unsigned)__cvta_generic_to_shared(p);
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %4, 0;\n\t"
+                 "@p ld.shared.v2.f64 {%0, %1}, [%5];\n\t@p ld.shared.v2.f64 {%2, %3}, [%5+16];\n\t}"
+                 : "+d"(a.re), "+d"(a.im), "+d"(b.re), "+d"(b.im) : "r"(take), "r"(addr) : "memory");
+}
 
-// One walk step, U = step index inside the M-step period.  fw / fr: this tile's outflow record and the right
-// neighbour's (entries 2U, 2U+1 of the current period).
+// ---- the exchange area -------------------------------------------------------------------------------------------
+// Per step every lane hands the pair phi_L(logical site 0), phi_L(logical site 1) to the lane below.  This goes through
+// shared memory, because there the FIFO costs nothing: addresses are per lane, so lane 0 simply writes its pair into the
+// outflow record instead of the exchange row, and lane 31 reads the inflow record instead of the exchange row — no
+// predicated instruction, no select, no register moves (warp shuffles cost 8 SHFL + about 12 MOV per step for
+// complex128, measured: FP64 instructions occupy the issue port for two cycles each, so every other instruction is
+// paid in FP64 time).  Addresses, in elements from the area base, for step t = s + U (U compile-time, s even):
+//     exchange rows   B0 = [0, 32), B1 = B0 + P                      step parity U & 1 picks the row (WAR safety)
+//     record a        [32, 32 + KMAX/2) for even t, + P for odd t     entry t at 32 + t/2 + (t & 1) * P
+//     record b        [32 + KMAX/2, 32 + KMAX), + P for odd t          (tiles alternate between a and b)
+// so every lane addresses  ptr + (U & 1) * P  with ptr a register that lane 0 / lane 31 bump by one element every
+// second step and the other lanes never.  The first amplitude of a pair lives in area 0, the second in area 1.
+// complex64 keeps the warp shuffles (4 SHFL per step and half as many FP instructions to hide them behind: measured
+// faster, 5.4e12 against 4.8e12 site-updates/s on K1): there lane 0 saves its pair to the record [j & 1][2k], then loads
+// the right-hand tile's pair into the same registers, and every lane takes the pair of lane + 1 (mod 32).
+template <typename R> struct Chain1dExchange {
+    static constexpr bool SMEM = sizeof(R) == 8;                  // exchange through shared memory (else shuffles)
+    static constexpr int KMAX = sizeof(R) == 8 ? 64 : 128;      // deepest launch the records hold
+    static constexpr int P = 32 + KMAX;                           // parity offset
+    static constexpr int AREA = 2 * P;                            // elements per area; two areas
+};
+
+// One walk step, U = step index inside the M-step period.
 template <typename R, int M, int KIND, int U>
-__device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C, int lane, bool has_in,
-                                             typename Cx<R>::T *fw, const typename Cx<R>::T *fr) {
+__device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
+                                             typename Cx<R>::T *&wptr, const typename Cx<R>::T *&rptr, int winc, int rinc) {
     typedef typename Cx<R>::T V;
+    typedef Chain1dExchange<R> EX;
 #pragma unroll
     for (int q = 0; q < M; ++q) {
         const int p = (q + 2 * U) % M;
@@ -73,29 +109,35 @@ __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M],
         Lp[p] = v[1];
     }
     // phi_L of logical sites 0 and 1 leaves the lane: it becomes L' of logical sites M-2, M-1 of the lane below
-    // (lane 0: of the tile to the left, through the FIFO); lane 31 receives what the tile to the right recorded.
     constexpr int P0 = (2 * U) % M, P1 = (2 * U + 1) % M;
-    const cplx<R> o0 = Lp[P0], o1 = Lp[P1];
-    if (lane == 0) {
-        V z0, z1;
-        z0.x = o0.re; z0.y = o0.im; z1.x = o1.re; z1.y = o1.im;
-        fw[2 * U] = z0; fw[2 * U + 1] = z1;
+    V z0, z1;
+    z0.x = Lp[P0].re; z0.y = Lp[P0].im; z1.x = Lp[P1].re; z1.y = Lp[P1].im;
+    if constexpr (EX::SMEM) {
+        constexpr int OFF = (U & 1) * EX::P;
+        wptr[OFF] = z0;
+        wptr[OFF + EX::AREA] = z1;
+        __syncwarp();
+        z0 = rptr[OFF];
+        z1 = rptr[OFF + EX::AREA];
+        Lp[P0] = cplx<R>{z0.x, z0.y};
+        Lp[P1] = cplx<R>{z1.x, z1.y};
+        if constexpr (U & 1) { wptr += winc; rptr += rinc; }      // lane 0 / lane 31: next pair of record entries
+    } else {
+        // winc != 0 marks lane 0; rinc = 1 if lane 0 takes a recorded inflow (not the starter), src lane in bits 8..
+        cplx<R> o0 = Lp[P0], o1 = Lp[P1];
+        if (winc) { wptr[2 * U] = z0; wptr[2 * U + 1] = z1; }
+        chain_fifo_load_in_place(rptr + 2 * U, (unsigned)(rinc & 1), o0, o1);
+        Lp[P0] = chain_shfl_from(o0, rinc >> 8);
+        Lp[P1] = chain_shfl_from(o1, rinc >> 8);
     }
-    cplx<R> i0 = chain_shfl_down1(o0), i1 = chain_shfl_down1(o1);
-    if (lane == 31 && has_in) {
-        const V z0 = fr[2 * U], z1 = fr[2 * U + 1];
-        i0 = cplx<R>{z0.x, z0.y}; i1 = cplx<R>{z1.x, z1.y};
-    }
-    Lp[P0] = i0;
-    Lp[P1] = i1;
 }
 
 template <typename R, int M, int KIND, int U>
 struct Chain1dUnroll {
-    static __device__ __forceinline__ void run(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C, int lane, bool has_in,
-                                               typename Cx<R>::T *fw, const typename Cx<R>::T *fr) {
-        chain1d_step<R, M, KIND, U>(Rp, Lp, C, lane, has_in, fw, fr);
-        if constexpr (U + 1 < M) Chain1dUnroll<R, M, KIND, U + 1>::run(Rp, Lp, C, lane, has_in, fw, fr);
+    static __device__ __forceinline__ void run(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
+                                               typename Cx<R>::T *&wptr, const typename Cx<R>::T *&rptr, int winc, int rinc) {
+        chain1d_step<R, M, KIND, U>(Rp, Lp, C, wptr, rptr, winc, rinc);
+        if constexpr (U + 1 < M) Chain1dUnroll<R, M, KIND, U + 1>::run(Rp, Lp, C, wptr, rptr, winc, rinc);
     }
 };
 
@@ -119,22 +161,34 @@ template <int M, int ES> __device__ __forceinline__ int chain_pos(int row, int c
 
 template <typename R, int M> struct Chain1dShape {
     // warps per CTA x CTAs per SM: complex128 8 warps per SM, complex64 16
-    static constexpr int WARPS = 4;
-    static constexpr int MINB = sizeof(R) == 8 ? 2 : 4;
+#ifndef QW_CHAIN_WARPS
+#define QW_CHAIN_WARPS 4
+#endif
+#ifndef QW_CHAIN_MINB64
+#define QW_CHAIN_MINB64 2
+#endif
+#ifndef QW_CHAIN_MINB32
+#define QW_CHAIN_MINB32 4
+#endif
+    static constexpr int WARPS = QW_CHAIN_WARPS;
+    static constexpr int MINB = sizeof(R) == 8 ? QW_CHAIN_MINB64 : QW_CHAIN_MINB32;
+    // shared memory of one warp, in elements: two prefetched input planes, HALF a plane of output staging, exchange
+    static constexpr int SMEM_ELEMS = 2 * 32 * M + 16 * M + 2 * Chain1dExchange<R>::AREA;
 };
 
 template <typename R, int M, int KIND>
 __global__ void __launch_bounds__(Chain1dShape<R, M>::WARPS * 32, Chain1dShape<R, M>::MINB)
 step_chain1d_kernel(const Chain1dArgs<R> a) {
     typedef typename Cx<R>::T V;
+    typedef Chain1dExchange<R> EX;
     constexpr int WARPS = Chain1dShape<R, M>::WARPS;
     constexpr int W = 32 * M;
+    constexpr int ES = (int)sizeof(V);
     extern __shared__ __align__(16) unsigned char chain_smem[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int per_warp = 3 * W + 4 * a.k;                                       // elements
-    V *st_in = reinterpret_cast<V *>(chain_smem) + (size_t)wid * per_warp;      // [2][W]: prefetched input planes
-    V *st_out = st_in + 2 * W;                                                  // [W]: output staging
-    V *fifo = st_out + W;                                                       // [2][2k]: outflow records
+    V *st_in = reinterpret_cast<V *>(chain_smem) + (size_t)wid * Chain1dShape<R, M>::SMEM_ELEMS;   // [2][W]: prefetched input planes
+    V *st_out = st_in + 2 * W;                                                  // [16][M]: output staging, half a plane
+    V *area = st_out + 16 * M;                                                  // [2][AREA]: exchange rows + outflow records
     const long long N = a.n_sites;
     const long long G = (long long)gridDim.x * WARPS;
 
@@ -146,7 +200,7 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
     // element i*32 + lane of a tile: row (i*32 + lane) / M, col (i*32 + lane) % M
     int pos_co[M];                                                              // coalesced-side staging positions
 #pragma unroll
-    for (int i = 0; i < M; ++i) pos_co[i] = chain_pos<M, (int)sizeof(V)>((i * 32 + lane) / M, (i * 32 + lane) % M);
+    for (int i = 0; i < M; ++i) pos_co[i] = chain_pos<M, ES>((i * 32 + lane) / M, (i * 32 + lane) % M);
 
     // chain -> (walk, first input site S, end E, number of tiles); tile j of a chain starts at E - j*W (j = 0: starter)
     auto chain_geom = [&](long long c, long long &w, long long &S, long long &E, int &nt) {
@@ -162,9 +216,9 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
         if (X >= 0 && X + W <= N) {
             const V *p0 = inw + X + lane, *p1 = p0 + a.plane_stride;
 #pragma unroll
-            for (int i = 0; i < M; ++i) chain_cp_async<(int)sizeof(V)>(st_in + pos_co[i], p0 + i * 32);
+            for (int i = 0; i < M; ++i) chain_cp_async<ES>(st_in + pos_co[i], p0 + i * 32);
 #pragma unroll
-            for (int i = 0; i < M; ++i) chain_cp_async<(int)sizeof(V)>(st_in + W + pos_co[i], p1 + i * 32);
+            for (int i = 0; i < M; ++i) chain_cp_async<ES>(st_in + W + pos_co[i], p1 + i * 32);
         } else {
 #pragma unroll 1
             for (int plane = 0; plane < 2; ++plane) {
@@ -173,8 +227,7 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
                     long long x = X + i * 32 + lane;
                     if (x < 0) x += N; else if (x >= N) x -= N;
                     const int e = i * 32 + lane;                 // run-time i: not through the register array pos_co
-                    chain_cp_async<(int)sizeof(V)>(st_in + plane * W + chain_pos<M, (int)sizeof(V)>(e / M, e % M),
-                                                   inw + plane * a.plane_stride + x);
+                    chain_cp_async<ES>(st_in + plane * W + chain_pos<M, ES>(e / M, e % M), inw + plane * a.plane_stride + x);
                 }
             }
         }
@@ -188,6 +241,9 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
         chain_geom(chain, w, S, E, nt);
         prefetch(w, E);
     }
+    // exchange pointers of this lane (see Chain1dExchange): lanes 1..31 write row entry `lane`, lanes 0..30 read row
+    // entry lane + 1; lane 0 writes and lane 31 reads the records, which alternate between a and b from tile to tile
+    const int winc = lane == 0 ? 1 : 0, rinc = lane == 31 ? 1 : 0;
     while (chain < a.total_chains) {
         for (int j = 0; j <= nt; ++j) {
             const long long X = E - (long long)j * W;
@@ -197,7 +253,7 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
             __syncwarp();
 #pragma unroll
             for (int i = 0; i < M; ++i) {
-                const V zr = st_in[chain_pos<M, (int)sizeof(V)>(lane, i)], zl = st_in[W + chain_pos<M, (int)sizeof(V)>(lane, i)];
+                const V zr = st_in[chain_pos<M, ES>(lane, i)], zl = st_in[W + chain_pos<M, ES>(lane, i)];
                 Rp[i] = cplx<R>{zr.x, zr.y};
                 Lp[i] = cplx<R>{zl.x, zl.y};
             }
@@ -210,44 +266,58 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
                 chain_geom(chain + G, w2, S2, E2, nt2);
                 prefetch(w2, E2);
             }
-            // ---- k steps in registers; the outflow of this tile feeds the next one (its left neighbour)
-            V *fw = fifo + (j & 1) * 2 * a.k;
-            const V *fr = fifo + ((j & 1) ^ 1) * 2 * a.k;
-            const bool has_in = j > 0;
-            for (int s = 0; s < a.k; s += M) {
-                Chain1dUnroll<R, M, KIND, 0>::run(Rp, Lp, C, lane, has_in, fw, fr);
-                fw += 2 * M; fr += 2 * M;
+            // ---- k steps in registers; the outflow of this tile is recorded for the next one (its left neighbour).
+            // The starter (j = 0) reads a record nobody wrote: its inflow is garbage by construction.
+            if constexpr (EX::SMEM) {
+                V *wptr = area + (lane == 0 ? 32 + (j & 1) * (EX::KMAX / 2) : lane);
+                const V *rptr = area + (lane == 31 ? 32 + ((j & 1) ^ 1) * (EX::KMAX / 2) : lane + 1);
+                for (int s = 0; s < a.k; s += M)
+                    Chain1dUnroll<R, M, KIND, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc);
+            } else {
+                V *wptr = area + (j & 1) * 2 * a.k;
+                const V *rptr = area + ((j & 1) ^ 1) * 2 * a.k;
+                const int rinc2 = (((lane + 1) & 31) << 8) | ((j > 0 && lane == 0) ? 1 : 0);
+                for (int s = 0; s < a.k; s += M) {
+                    Chain1dUnroll<R, M, KIND, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc2);
+                    wptr += 2 * M; rptr += 2 * M;
+                }
+                __syncwarp();                              // outflow record complete before the next tile reads it
             }
-            __syncwarp();                                  // outflow record complete before the next tile reads it
             if (j == 0) continue;                          // the starter stores nothing
-            // ---- store: element e of the tile is output site X + k + e; this chain owns input coordinates >= S
+            // ---- store: element e of the tile is output site X + k + e; this chain owns input coordinates >= S.
+            // Registers -> swizzled shared -> coalesced global, half a plane (the rows of 16 lanes) at a time.
             const bool whole = X >= S && X + a.k + W <= N;
-            const long long xo = X + a.k + lane;           // output coordinate of element `lane` (unwrapped)
 #pragma unroll
             for (int plane = 0; plane < 2; ++plane) {
-#pragma unroll
-                for (int i = 0; i < M; ++i) {
-                    V z;
-                    if (plane == 0) { z.x = Rp[i].re; z.y = Rp[i].im; } else { z.x = Lp[i].re; z.y = Lp[i].im; }
-                    st_out[chain_pos<M, (int)sizeof(V)>(lane, i)] = z;
-                }
-                __syncwarp();
                 V *op = a.out + w * a.walk_stride + plane * a.plane_stride;
-                if (whole) {
 #pragma unroll
-                    for (int i = 0; i < M; ++i) op[xo + i * 32] = st_out[pos_co[i]];
-                } else {
+                for (int h = 0; h < 2; ++h) {
+                    __syncwarp();
+                    if ((lane >> 4) == h) {
+#pragma unroll
+                        for (int i = 0; i < M; ++i) {
+                            V z;
+                            if (plane == 0) { z.x = Rp[i].re; z.y = Rp[i].im; } else { z.x = Lp[i].re; z.y = Lp[i].im; }
+                            st_out[chain_pos<M, ES>(lane & 15, i)] = z;
+                        }
+                    }
+                    __syncwarp();
+                    const long long xo = X + a.k + h * (16 * M) + lane;      // output coordinate of half-plane element `lane`
+                    if (whole) {
+#pragma unroll
+                        for (int i = 0; i < M / 2; ++i) op[xo + i * 32] = st_out[pos_co[i]];
+                    } else {
 #pragma unroll 4
-                    for (int i = 0; i < M; ++i) {
-                        long long x = xo + i * 32;
-                        if (x - a.k >= S) {
-                            if (x >= N) x -= N;
-                            const int e = i * 32 + lane;
-                            op[x] = st_out[chain_pos<M, (int)sizeof(V)>(e / M, e % M)];
+                        for (int i = 0; i < M / 2; ++i) {
+                            long long x = xo + i * 32;
+                            if (x - a.k >= S) {
+                                if (x >= N) x -= N;
+                                const int e = i * 32 + lane;
+                                op[x] = st_out[chain_pos<M, ES>(e / M, e % M)];
+                            }
                         }
                     }
                 }
-                __syncwarp();
             }
         }
         chain += G;
@@ -258,8 +328,12 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
 // ---- host side ---------------------------------------------------------------------------------------------------
 
 int chain1d_granule(const qw_sim *s) { return s->coin_kind == COIN_HADAMARD ? 16 : 8; }
-constexpr int CHAIN1D_MAX_K = 64;       // FIFO size (4 k elements of shared memory per warp); also <= W/2 = 16*M
-int chain1d_max_k(const qw_sim *) { return CHAIN1D_MAX_K; }
+// deepest launch: what the outflow records hold (Chain1dExchange::KMAX), and k <= W/2 = 16*M for the starter tile
+int chain1d_max_k(const qw_sim *s) {
+    const int kmax = s->dtype == QW_C128 ? Chain1dExchange<double>::KMAX : Chain1dExchange<float>::KMAX;
+    const int half = 16 * chain1d_granule(s);
+    return kmax < half ? kmax : half;
+}
 
 // Resident warps of the grid and the dynamic shared memory of one CTA at depth k.  The kernel attribute and the
 // occupancy are taken once per device for the deepest launch, so every depth runs with the same persistent grid.
@@ -267,7 +341,7 @@ template <typename R, int M, int KIND>
 static int chain1d_grid(const qw_sim *s, int k, int *warps_out, size_t *smem_out) {
     typedef typename Cx<R>::T V;
     constexpr int WARPS = Chain1dShape<R, M>::WARPS;
-    const size_t smem_max = (size_t)WARPS * (3 * 32 * M + 4 * CHAIN1D_MAX_K) * sizeof(V);
+    const size_t smem_max = (size_t)WARPS * Chain1dShape<R, M>::SMEM_ELEMS * sizeof(V);
     auto kern = step_chain1d_kernel<R, M, KIND>;
     static int ctas_per_sm[64];                                            // per device (cudaFuncSetAttribute is per device)
     const int dev = s->device & 63;
@@ -281,7 +355,7 @@ static int chain1d_grid(const qw_sim *s, int k, int *warps_out, size_t *smem_out
         ctas_per_sm[dev] = n;
     }
     *warps_out = s->sm_count * ctas_per_sm[dev] * WARPS;
-    *smem_out = (size_t)WARPS * (3 * 32 * M + 4 * k) * sizeof(V);
+    *smem_out = smem_max;
     return ctas_per_sm[dev];
 }
 
