@@ -78,7 +78,7 @@ __device__ __forceinline__ void chain_fifo_load_in_place(const double2 *p, unsig
 // the right-hand tile's pair into the same registers, and every lane takes the pair of lane + 1 (mod 32).
 template <typename R> struct Chain1dExchange {
     static constexpr bool SMEM = sizeof(R) == 8;                  // exchange through shared memory (else shuffles)
-    static constexpr int KMAX = sizeof(R) == 8 ? 64 : 128;      // deepest launch the records hold
+    static constexpr int KMAX = sizeof(R) == 8 ? 96 : 128;      // deepest launch the records hold
     static constexpr int P = 32 + KMAX;                           // parity offset
     static constexpr int AREA = 2 * P;                            // elements per area; two areas
 };
@@ -160,7 +160,7 @@ template <int M, int ES> __device__ __forceinline__ int chain_pos(int row, int c
 }
 
 template <typename R, int M> struct Chain1dShape {
-    // warps per CTA x CTAs per SM: complex128 8 warps per SM, complex64 16
+    // warps per CTA x CTAs per SM: complex128 8 warps per SM, complex64 12 (measured: 16 warps at 128 registers are slower)
 #ifndef QW_CHAIN_WARPS
 #define QW_CHAIN_WARPS 4
 #endif
@@ -168,12 +168,13 @@ template <typename R, int M> struct Chain1dShape {
 #define QW_CHAIN_MINB64 2
 #endif
 #ifndef QW_CHAIN_MINB32
-#define QW_CHAIN_MINB32 4
+#define QW_CHAIN_MINB32 3
 #endif
     static constexpr int WARPS = QW_CHAIN_WARPS;
     static constexpr int MINB = sizeof(R) == 8 ? QW_CHAIN_MINB64 : QW_CHAIN_MINB32;
     // shared memory of one warp, in elements: two prefetched input planes, HALF a plane of output staging, exchange
-    static constexpr int SMEM_ELEMS = 2 * 32 * M + 16 * M + 2 * Chain1dExchange<R>::AREA;
+    static constexpr int SMEM_ELEMS = 2 * 32 * M + 16 * M +
+        (Chain1dExchange<R>::SMEM ? 2 * Chain1dExchange<R>::AREA : 4 * Chain1dExchange<R>::KMAX);
 };
 
 template <typename R, int M, int KIND>
