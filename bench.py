@@ -54,6 +54,13 @@ def make_workload(name: str, walk_steps=None):
         return qi.k4(steps=walk_steps)
     if name == "k0":
         return qi.k0(steps=walk_steps or 100)
+    if name == "seg":
+        # NEXT-3: the paper's Fig. 3-left "segment": an open 1D Hadamard segment with
+        # the delta start of K0, run for five times its length so that the front reflects off the walls (A3, PAPER.md:94-101
+        # with RBL = 0) about ten times.  Parity-tested at full length (tests/test_parity_gpu.py::test_segment_workload).
+        w = qi.k0(steps=walk_steps or 10000, half_width=1000)
+        w.name = "SEG"
+        return w
     if name == "t1":
         # context only: the largest row of the paper's Table 1 (1D segment of size 10000).  The paper
         # does not state the number of iterations; iterations = size is SURVEY.md section 6's conjecture.
@@ -88,7 +95,7 @@ def workload_config(name, w, extra=None):
     return cfg
 
 
-def coin_cost(w, sched_name="fused"):
+def coin_cost(w, sched_name="fused", kdepth=0):
     """(instructions, flops) per site-step of the coin arithmetic the named schedule executes for this workload
     (csrc/qw_coin.cuh::apply_coin; DESIGN.md section 5): mul = 1 flop, fma = 2 flops, add = 1 flop.
     The temporally blocked 1D kernel defers the Hadamard scale: 15 bare butterflies (4 add) + 1 scaled step
@@ -104,7 +111,7 @@ def coin_cost(w, sched_name="fused"):
         return instr, flops
     # 2D named coins: scaled evaluation 20 / 16 / 20 instructions; the tiled kernel defers the power-of-two scale:
     # K-1 bare steps (H(x)H, DFT: 16 add; Grover: 6 add + 8 fma) + 1 scaled step per K steps
-    K = 8 if w.dtype == np.complex64 else 6
+    K = kdepth if kdepth in (2, 4, 6, 8) else (8 if w.dtype == np.complex64 else 6)
     def tiled(bare_i, bare_f, full_i, full_f):
         if sched_name == "tiled":
             return ((K - 1) * bare_i + full_i) / K, ((K - 1) * bare_f + full_f) / K
@@ -249,43 +256,69 @@ def aggregate_rate(units_per_rank: float, ms_per_rank: float, world: int, device
 
 
 # ----------------------------------------------------------------------------------------------
-def oracle_sample(name: str, w, seconds_target: float = 12.0):
-    """Time the CPU oracle, as it stands, on a bounded sample of workload `name` (1 thread)."""
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+class pinned_to_one_core:
+    """the oracle is timed on ONE host core (what `taskset -c <core>` does)."""
+    def __enter__(self):
+        self.old = None
+        try:
+            self.old = os.sched_getaffinity(0)
+            self.core = min(self.old)
+            os.sched_setaffinity(0, {self.core})
+        except (AttributeError, OSError):
+            self.core = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.old is not None:
+            try:
+                os.sched_setaffinity(0, self.old)
+            except OSError:
+                pass
+
+
+def oracle_sample(name: str, w, seconds_target: float = 15.0):
+    """Time the CPU oracle, as it stands, on a bounded sample of workload `name`: the FULL lattice of the config
+     for a few walk steps (about `seconds_target` seconds), one thread pinned to one core."""
     import oracle
     oracle.build()
-    if name in ("k1", "k1c64"):
-        sw = qi.k1(log2_sites=22, steps=8, dtype=w.dtype)
-        desc = "same ring workload cut to 2^22 sites x %d walk steps"
-    elif name == "k2":
-        sw = qi.k2(half=512, steps=4)
-        desc = "same open Grover lattice cut to 1025^2 sites x %d walk steps"
-    elif name in ("k3hxh", "k3dft"):
-        sw = qi.k3(extent=1024, steps=4, coin=name[2:])
-        desc = "same torus workload cut to 1024^2 sites x %d walk steps"
-    elif name == "k4":
-        sw = qi.k4(batch=64, half=1024, steps=32)
-        desc = "64 of the 4096 walks x %d walk steps"
-    elif name in ("t1", "t2"):
-        sw = make_workload(name, 8)
-        desc = "the same lattice, %d walk steps"
+    sw = w
+    if name == "k4":
+        sw = qi.k4(batch=256, half=1024, steps=1)        # the per-site matrices of all 4096 walks would be 537 MB x 2
+        desc = "256 of the 4096 walks, full length of each, %d walk steps"
+    elif name in ("k0", "seg", "t1"):
+        desc = "the whole lattice, %d walk steps"
     else:
-        sw = qi.k0()
-        desc = "the whole config (%d walk steps)"
+        desc = "the FULL lattice of the config, %d walk steps"
     mode, coin = sw.general_coin_f64()
     psi = np.ascontiguousarray(sw.initial_state().astype(np.complex128))
+    if sw.state is None:                                     # delta start: spread the walker first (cost is per site anyway)
+        psi[:] = 1.0 / np.sqrt(psi.size)
     kw = dict(boundary=sw.boundary, coin_mode=mode, batch=sw.batch, lattice=sw.lattice)
-    # calibrate: one short call, then scale the step count to ~seconds_target
-    t0 = time.perf_counter(); oracle.step(sw.extents, coin, psi, 1, **kw); t1 = time.perf_counter() - t0
-    steps = int(max(1, min(4096, seconds_target / max(t1, 1e-6))))
-    t0 = time.perf_counter(); oracle.step(sw.extents, coin, psi, steps, **kw); dt = time.perf_counter() - t0
-    if "probabilities" in sw.outputs:
-        oracle.probabilities(sw.extents, psi, batch=sw.batch)
-    if "moments" in sw.outputs:
-        oracle.moments(sw.extents, psi, batch=sw.batch)
+    with pinned_to_one_core() as pin:
+        # calibrate: one step, then scale the step count to ~seconds_target
+        t0 = time.perf_counter(); oracle.step(sw.extents, coin, psi, 1, **kw); t1 = time.perf_counter() - t0
+        steps = int(max(1, min(100000, seconds_target / max(t1, 1e-7))))
+        t0 = time.perf_counter(); oracle.step(sw.extents, coin, psi, steps, **kw); dt = time.perf_counter() - t0
+        if "probabilities" in sw.outputs:
+            oracle.probabilities(sw.extents, psi, batch=sw.batch)
+        if "moments" in sw.outputs:
+            oracle.moments(sw.extents, psi, batch=sw.batch)
     rate = sw.sites * sw.batch * steps / dt
     return {"value": rate, "unit": METRIC, "cores": 1, "kind": "oracle",
-            "sample": (desc % steps) + ", single thread, g++ -O2 (oracle/qw_oracle.cpp)",
-            "seconds": dt, "host_cores_available": os.cpu_count()}
+            "sample": (desc % steps) + ", single thread pinned to core %s (sched_setaffinity = taskset -c), g++ -O2 "
+                      "-ffp-contract=off (oracle/qw_oracle.cpp)" % pin.core,
+            "seconds": dt, "cpu_model": cpu_model(), "host_cores_available": os.cpu_count()}
 
 
 def run_reference(args):
@@ -293,9 +326,6 @@ def run_reference(args):
     rank, world, _ = dist_env()
     if rank != 0:
         return 0
-    w_desc = make_workload(args.workload, args.walk_steps) if args.workload in ("k0",) else None
-    # describe the workload without materialising the 2 GiB state
-    names = {"k1": ("K1", 1, (1 << 26,), 1, np.complex128, 1000), "k1c64": ("K1", 1, (1 << 26,), 1, np.complex64, 1000)}
     import oracle
     oracle.build()
     if args.workload in ("k1", "k1c64"):
@@ -307,13 +337,14 @@ def run_reference(args):
     else:
         sw = {"k2": lambda: qi.k2(half=512, steps=2), "k3hxh": lambda: qi.k3(extent=1024, steps=2, coin="hxh"),
               "k3dft": lambda: qi.k3(extent=1024, steps=2, coin="dft"), "k4": lambda: qi.k4(batch=64, steps=16),
-              "k0": lambda: qi.k0()}[args.workload]()
+              "k0": lambda: qi.k0(), "seg": lambda: make_workload("seg", 1000),
+              "t1": lambda: make_workload("t1", 8), "t2": lambda: make_workload("t2", 8)}[args.workload]()
         sample = "%s cut to %d sites x batch %d, %d walk steps per bench step" % (sw.name, sw.sites, sw.batch, sw.steps)
         full_sites, full_batch, full_steps = sw.sites, sw.batch, sw.steps
         wl_name = sw.name
     mode, coin = sw.general_coin_f64()
     psi = np.ascontiguousarray(sw.initial_state().astype(np.complex128))
-    kw = dict(boundary=sw.boundary, coin_mode=mode, batch=sw.batch)
+    kw = dict(boundary=sw.boundary, coin_mode=mode, batch=sw.batch, lattice=sw.lattice)
 
     def one():
         oracle.step(sw.extents, coin, psi, sw.steps, **kw)
@@ -322,21 +353,25 @@ def run_reference(args):
         if "probabilities" in sw.outputs:
             oracle.probabilities(sw.extents, psi, batch=sw.batch)
 
-    for _ in range(args.warmup):
-        one()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        one()
-    dt = time.perf_counter() - t0
+    if args.steps is None:
+        args.steps = 3
+    with pinned_to_one_core() as pin:
+        for _ in range(args.warmup):
+            one()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            one()
+        dt = time.perf_counter() - t0
     rate = sw.sites * sw.batch * sw.steps * args.steps / dt
     line = {
         "impl": "reference", "metric": METRIC, "value": rate, "unit": METRIC, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s (BASELINE.json configs[%d]); reference arm = CPU oracle on a bounded sample: %s"
-                               % (wl_name, {"k0": 0, "k1": 1, "k1c64": 1, "k2": 2, "k3hxh": 3, "k3dft": 3, "k4": 4}[args.workload], sample),
+                               % (wl_name, {"k0": 0, "k1": 1, "k1c64": 1, "k2": 2, "k3hxh": 3, "k3dft": 3, "k4": 4}.get(args.workload, -1), sample),
                    "sites": full_sites, "batch": full_batch, "walk_steps": full_steps, "parallelism": "replicas"},
-        "cpu_baseline": {"value": rate, "unit": METRIC, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": rate, "unit": METRIC, "cores": 1, "kind": "oracle", "cpu_model": cpu_model(),
+                         "sample": sample + "; one thread pinned to core %s" % pin.core},
         "e2e": {"value": rate, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -404,17 +439,30 @@ def run_gpu(args):
             qw.qw_set_state_delta(h, w.delta_site, delta_coin)
         qw.qw_step(h, w.steps)
 
+    # measured plain-ALU peak of this device (register-only DADD / DFMA / FADD2 / FFMA2 chains on every SM,
+    # csrc/qw_peak.cu): the denominator of the roofline of the schedules that are not HBM-bound
+    dcode = qw.dtype_code(w.dtype)
+    alu_measured = {"add": qw.qw_measure_alu_peak(dcode, qw.QW_PEAK_ADD), "fma": qw.qw_measure_alu_peak(dcode, qw.QW_PEAK_FMA)}
+
     qw.load_state(h, w)
     for _ in range(max(args.warmup, 3)):
         hot_path()
         outputs_device()
     torch.cuda.synchronize()
+    if args.steps is None:
+        # as many bench steps as make the timed region last about 2 s (>= 10 clock samples at 100 ms), at least 3
+        ca = torch.cuda.Event(enable_timing=True); cb = torch.cuda.Event(enable_timing=True)
+        ca.record(stream); hot_path(); outputs_device(); cb.record(stream)
+        torch.cuda.synchronize()
+        one_ms = max_over_ranks(ca.elapsed_time(cb), world, dev)
+        args.steps = int(max(3, min(100000, np.ceil(2000.0 / max(one_ms, 1e-3)))))
     barrier(world)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
     l0 = qw.qw_get_info(h, qw.QW_INFO_LAUNCHES)
+    touched0 = qw.qw_get_info(h, qw.QW_INFO_SITES_TOUCHED)
     torch.cuda.synchronize()
     for i in range(args.steps):
         ev[i][0].record(stream)
@@ -426,6 +474,7 @@ def run_gpu(args):
     barrier(world)
     clocks = sampler.stop() if rank == 0 else None
     launches = qw.qw_get_info(h, qw.QW_INFO_LAUNCHES) - l0
+    touched_per_step = (qw.qw_get_info(h, qw.QW_INFO_SITES_TOUCHED) - touched0) / float(args.steps)
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
     step_ms = sum(e[0].elapsed_time(e[1]) for e in ev)
     out_ms = sum(e[1].elapsed_time(e[2]) for e in ev)
@@ -456,7 +505,7 @@ def run_gpu(args):
 
         e2e_step()
         torch.cuda.synchronize(); barrier(world)
-        n_e2e = max(1, min(args.steps, 3))
+        n_e2e = max(1, min(args.steps, 3 if h2d > (1 << 28) else 50))
         t0 = time.perf_counter()
         a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
         a.record(stream)
@@ -499,33 +548,46 @@ def run_gpu(args):
     kname = {1: "step_scatter_kernel (generic)", 2: "step_scatter_kernel (fused coin+shift)",
              3: "step_blocked1d_kernel" if w.dim == 1 else "step_blocked2d_kernel", 4: "step_resident1d_kernel",
              5: "step_tiled2d_kernel"}.get(sched, "?")
+    touched_frac = touched_per_step / site_updates_per_step          # < 1 when the light-cone window skipped work
     if sched in (1, 2):
+        touched_gbs = eff_gbs * touched_frac
         roofline = {
-            "bound": "hbm", "kernel": kname, "achieved": eff_gbs, "peak": peak, "unit": "GB/s", "frac": eff_gbs / peak,
-            "peak_source": "of " + peak_src, "frac_of_nominal_8000": eff_gbs / 8000.0,
+            "bound": "hbm", "kernel": kname, "achieved": touched_gbs, "peak": peak, "unit": "GB/s", "frac": touched_gbs / peak,
+            "peak_source": "of " + peak_src, "frac_of_nominal_8000": touched_gbs / 8000.0,
+            "effective_achieved": eff_gbs, "effective_frac": eff_gbs / peak,
             "algorithmic_bytes_per_site_step": alg_bytes_per_site,
             "avg_launch_ms": step_ms / (w.steps * args.steps),
             "traffic": stored_traffic(args.workload),
-            "note": "achieved = 2*coin_dim*sizeof(complex) B x site-updates / CUDA-event time of qw_step (launch gaps included)"
-                    + ("; light-cone window active: site-updates are counted on the FULL lattice, so this is an effective figure" if windowed else ""),
+            "note": "achieved = 2*coin_dim*sizeof(complex) B x site-updates the kernels produced (QW_INFO_SITES_TOUCHED) / CUDA-event "
+                    "time of qw_step (launch gaps included); effective_* counts the FULL lattice (BASELINE.json:metric)",
         }
     else:
-        instr, flops = coin_cost(w, sched_name)
-        ipeak = alu_peak(w, clocks["sm_max_mhz"] if clocks else None)
-        rate = site_updates_per_step / (kernel_ms * 1e-3)
+        instr, flops = coin_cost(w, sched_name, kdepth)
+        ipeak_derived = alu_peak(w, clocks["sm_max_mhz"] if clocks else None)
+        ipeak = alu_measured["add"] if alu_measured["add"] > 0 else ipeak_derived
+        rate = site_updates_per_step / (kernel_ms * 1e-3)         # full lattice (the metric)
+        rate_touched = rate * touched_frac                        # what the kernels computed
         fpi = flops / instr                      # flops per instruction of this kernel's op mix (add/mul 1, fma 2)
         roofline = {
-            "bound": "alu", "kernel": kname, "achieved": rate * flops / 1e12, "peak": ipeak * fpi / 1e12, "unit": "TFLOP/s",
-            "frac": rate * instr / ipeak,
-            "frac_of_fma_peak": rate * flops / (2 * ipeak), "fma_peak": 2 * ipeak / 1e12,
-            "peak_source": "derived: 148 SMs x %d %s lanes x sm_max_mhz instruction slots/s x %.3f flops per instruction of "
-                           "this kernel's arithmetic (add/mul = 1, fma = 2; DESIGN.md section 5)"
-                           % (64 if w.dtype == np.complex128 else 128, "FP64" if w.dtype == np.complex128 else "FP32", fpi),
+            "bound": "alu", "kernel": kname, "achieved": rate_touched * flops / 1e12, "peak": ipeak * fpi / 1e12, "unit": "TFLOP/s",
+            "frac": rate_touched * instr / ipeak,
+            "effective_frac": rate * instr / ipeak,
+            "peak_source": "measured: qw_measure_alu_peak (csrc/qw_peak.cu), independent %s chains on all SMs = %.4g thread-level "
+                           "instructions/s (%s: %.4g), x %.3f flops per instruction of this kernel's arithmetic (add/mul = 1, fma = 2)"
+                           % ("DADD" if w.dtype == np.complex128 else "FADD2", alu_measured["add"],
+                              "DFMA" if w.dtype == np.complex128 else "FFMA2", alu_measured["fma"], fpi),
+            "peak_derived": ipeak_derived * fpi / 1e12, "frac_of_derived_peak": rate_touched * instr / ipeak_derived,
+            "peak_derived_source": "148 SMs x %d %s lanes x sm_max_mhz (B200_PROFILING.md / B300_MICROARCH.md unit counts)"
+                                   % (64 if w.dtype == np.complex128 else 128, "FP64" if w.dtype == np.complex128 else "FP32"),
+            "frac_of_fma_peak": rate_touched * flops / (2 * alu_measured["fma"]) if alu_measured["fma"] > 0 else None,
+            "fma_peak": 2 * alu_measured["fma"] / 1e12,
             "algorithmic_flops_per_site_step": flops, "algorithmic_instr_per_site_step": instr,
+            "touched_site_updates_per_bench_step": touched_per_step, "touched_fraction_of_full_lattice": touched_frac,
             "traffic": stored_traffic(args.workload + "_" + sched_name),
             "effective_hbm_gbs_vs_single_step": eff_gbs, "single_step_hbm_roofline_x": eff_gbs / peak,
-            "note": "temporal blocking / SM residency removes the HBM bound; algorithmic work excludes halo recomputation"
-                    + ("; light-cone window active: counted on the FULL lattice (effective)" if windowed else ""),
+            "note": "temporal blocking / SM residency removes the HBM bound; frac counts the FP instructions of the site-updates the "
+                    "kernels produced (halo / starter recomputation excluded; with the light-cone window only the tiles and warps "
+                    "that were not skipped), effective_frac counts the full lattice (BASELINE.json:metric)",
         }
     if fused is not None:
         fg = fused["site_updates_per_s"] * alg_bytes_per_site / 1e9
@@ -544,10 +606,16 @@ def run_gpu(args):
         "roofline": roofline,
         "fused_single_step": fused,
         "clocks": clocks,
+        "alu_peak_measured": {"add_ops_per_s": alu_measured["add"], "fma_ops_per_s": alu_measured["fma"],
+                              "how": "qw_measure_alu_peak: register-only chains, 8 CTAs x 256 threads per SM, best of 4"},
         "gpu_launches": int(launches),
         "e2e": e2e,
         "result": {"norm": float(mom_host[0, 0]), "mean": float(mom_host[0, 1]), "var": float(mom_host[0, -1] if w.dim == 1 else mom_host[0, 3])},
     }
+    if clocks is not None and (clocks.get("samples") or 0) < 3:
+        # a timed region shorter than a few sampler periods has no clock record: not a result (use more --steps)
+        line["invalid"] = "only %d clock samples during the timed region (%.0f ms): rerun with more --steps" % (
+            clocks.get("samples") or 0, ms)
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = oracle_sample(args.workload, w)
     elif world > 1:
@@ -556,13 +624,23 @@ def run_gpu(args):
     return 0
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` outside torchrun: start the N ranks ourselves (one process per GPU) with the very
+    command line the driver uses, and hand its exit code back.  Rank 0 of the child job prints the JSON line."""
+    port = 29500 + os.getpid() % 2000
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=None,
+                    help="timed bench steps (default: as many as make the timed region last about 2 s, at least 3)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="k1", choices=["k0", "k1", "k1c64", "k2", "k3hxh", "k3dft", "k4", "t1", "t2"])
+    ap.add_argument("--workload", default="k1", choices=["k0", "k1", "k1c64", "k2", "k3hxh", "k3dft", "k4", "seg", "t1", "t2"])
     ap.add_argument("--walk-steps", type=int, default=None, help="walk steps per bench step (default: the config's)")
     ap.add_argument("--schedule", default=None, choices=["auto", "generic", "fused", "blocked", "resident", "tiled"])
     ap.add_argument("--k", type=int, default=0)
@@ -575,6 +653,10 @@ def main():
     ap.add_argument("--no-fused-leg", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args)
+    if args.gpus != int(os.environ.get("WORLD_SIZE", "1")):
+        raise SystemExit("--gpus %d does not match WORLD_SIZE=%s" % (args.gpus, os.environ.get("WORLD_SIZE")))
     if args.impl == "reference":
         return run_reference(args)
     return run_gpu(args)

@@ -85,7 +85,10 @@ enum {
     QW_INFO_LAST_SCHEDULE = 2,  /* schedule the last qw_step actually used (QW_SCHED_*)                   */
     QW_INFO_LAST_K = 3,         /* temporal block depth of the last qw_step (1 if not blocked)           */
     QW_INFO_STATE_BYTES = 4,    /* bytes of one device state buffer (there are two)                      */
-    QW_INFO_WINDOW = 5          /* 1 if the light-cone window is active                                  */
+    QW_INFO_WINDOW = 5,         /* 1 if the light-cone window is active                                  */
+    QW_INFO_SITES_TOUCHED = 6   /* site-steps the kernels were asked to produce so far: with the light-cone
+                                   window only the sites / tiles / warps that were not skipped count; halo
+                                   recomputation does not.  Without a window = batch * sites * steps          */
 };
 
 /* qw_set_option keys */
@@ -186,6 +189,16 @@ int qw_set_window(qw_sim *s, int enable);
 int qw_set_option(qw_sim *s, int key, int64_t value);
 
 int qw_get_info(const qw_sim *s, int what, int64_t *out);
+
+/* Diagnostic for the roofline of the schedules that are not HBM-bound (temporally blocked, resident): the measured
+ * plain-ALU throughput of the current device for the instructions the coin arithmetic is made of (PAPER.md:37-38
+ * eq. 1 evaluated as additions and fused multiply-adds, csrc/qw_coin.cuh).  dtype QW_C128: FP64 (DADD / DFMA);
+ * QW_C64: packed FP32x2 (FADD2 / FFMA2).  op: QW_PEAK_ADD or QW_PEAK_FMA.  Runs a register-only kernel on every
+ * SM of the current device (default stream, synchronous, a few milliseconds) and stores thread-level operations per
+ * second (an FMA counts as ONE operation, a packed instruction as two) in *ops_per_second (host pointer).
+ * No handle, no walk arithmetic. */
+enum { QW_PEAK_ADD = 0, QW_PEAK_FMA = 1 };
+int qw_measure_alu_peak(int dtype, int op, double *ops_per_second);
 
 /* Block the host until the handle's stream is idle; reports asynchronous CUDA errors. */
 int qw_synchronize(const qw_sim *s);

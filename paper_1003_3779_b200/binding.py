@@ -21,7 +21,8 @@ QW_PERIODIC, QW_OPEN = 0, 1
 QW_NATURAL, QW_DIAGONAL = 0, 1
 QW_COIN_UNIFORM, QW_COIN_PER_WALK, QW_COIN_PER_SITE = 0, 1, 2
 QW_SCHED_AUTO, QW_SCHED_GENERIC, QW_SCHED_FUSED, QW_SCHED_BLOCKED, QW_SCHED_RESIDENT, QW_SCHED_TILED = 0, 1, 2, 3, 4, 5
-QW_INFO_LAUNCHES, QW_INFO_TIME, QW_INFO_LAST_SCHEDULE, QW_INFO_LAST_K, QW_INFO_STATE_BYTES, QW_INFO_WINDOW = range(6)
+QW_INFO_LAUNCHES, QW_INFO_TIME, QW_INFO_LAST_SCHEDULE, QW_INFO_LAST_K, QW_INFO_STATE_BYTES, QW_INFO_WINDOW, \
+    QW_INFO_SITES_TOUCHED = range(7)
 QW_OPT_MAX_CTAS, QW_OPT_BLOCKED1D_KERNEL = 0, 1
 
 # every symbol include/qw.h declares (tests/test_abi.py checks the header against this list)
@@ -29,7 +30,7 @@ SYMBOLS = (
     "qw_create", "qw_create_batch", "qw_destroy", "qw_set_stream", "qw_set_lattice", "qw_set_coin",
     "qw_set_site_phases", "qw_set_broken_links", "qw_set_random_broken_links", "qw_set_state", "qw_set_state_delta", "qw_get_state",
     "qw_step", "qw_step_inverse", "qw_probabilities", "qw_moments", "qw_set_schedule", "qw_set_window",
-    "qw_set_option", "qw_get_info", "qw_synchronize", "qw_last_error",
+    "qw_set_option", "qw_get_info", "qw_measure_alu_peak", "qw_synchronize", "qw_last_error",
 )
 
 
@@ -75,6 +76,7 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
         "qw_set_window": [vp, ci],
         "qw_set_option": [vp, ci, i64],
         "qw_get_info": [vp, ci, i64p],
+        "qw_measure_alu_peak": [ci, ci, ctypes.POINTER(ctypes.c_double)],
         "qw_synchronize": [vp],
     }
     for name, args in sig.items():
@@ -201,6 +203,15 @@ def qw_set_option(h, key, value) -> None:
 def qw_get_info(h, what) -> int:
     out = ctypes.c_int64()
     _check(load().qw_get_info(h, what, ctypes.byref(out)))
+    return out.value
+
+
+QW_PEAK_ADD, QW_PEAK_FMA = 0, 1
+
+
+def qw_measure_alu_peak(dtype, op) -> float:
+    out = ctypes.c_double()
+    _check(load().qw_measure_alu_peak(int(dtype), int(op), ctypes.byref(out)))
     return out.value
 
 

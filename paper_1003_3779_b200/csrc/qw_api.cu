@@ -419,6 +419,7 @@ int qw_step(qw_sim *s, int64_t n) {
             const int kk = (int)(remaining >= kmax ? kmax : remaining);
             int rc = launch_step_blocked2d(s, s->cur, 1 - s->cur, kk);
             if (rc) return rc;
+            s->touched += (double)s->g.batch * (double)s->g.sites * kk;
             s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;
         }
         return QW_OK;
@@ -454,9 +455,11 @@ int qw_step(qw_sim *s, int64_t n) {
             if (chain && remaining >= M) {
                 kk = (int)(remaining >= kchain ? kchain : remaining / M * M);
                 rc = launch_step_chain1d(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), kk);
+                if (!rc) s->touched += (double)s->g.batch * (double)s->g.sites * kk;
             } else {
                 kk = remaining >= M ? (int)(remaining >= kmax ? kmax : remaining / M * M) : (remaining >= 8 ? 8 : 4);
                 rc = launch_step_blocked1d(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), kk);
+                if (!rc) s->touched += (double)s->g.batch * (double)s->g.sites * kk;
             }
             if (rc) return rc;
             s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;
@@ -467,6 +470,7 @@ int qw_step(qw_sim *s, int64_t n) {
         const Box box = step_box(s);
         int rc = launch_step(s, state_ptr(s, s->cur), state_ptr(s, 1 - s->cur), box, allow_fast);
         if (rc) return rc;
+        s->touched += (double)s->g.batch * (double)(box.m_hi - box.m_lo + 1) * (double)(box.n_hi - box.n_lo + 1);
         s->cur ^= 1; s->t += 1; s->radius += 1;
     }
     return QW_OK;
@@ -566,6 +570,7 @@ int qw_get_info(const qw_sim *s, int what, int64_t *out) {
         case QW_INFO_LAST_K: *out = s->last_k; break;
         case QW_INFO_STATE_BYTES: *out = (int64_t)s->state_bytes; break;
         case QW_INFO_WINDOW: *out = (s->window_enabled && s->window_valid) ? 1 : 0; break;
+        case QW_INFO_SITES_TOUCHED: *out = (int64_t)s->touched; break;
         default: return fail(QW_EINVAL, "unknown info key %d", what);
     }
     return QW_OK;

@@ -87,6 +87,9 @@ struct qw_sim {
     int sched, sched_k;
     int last_sched, last_k;
     long long launches;
+    double touched;          // site-steps the kernels were asked to produce so far (QW_INFO_SITES_TOUCHED): the sites
+                             // inside the light-cone window / the tiles and warps that were not skipped; halo
+                             // recomputation is not counted
 
     // TMA descriptors of the two state buffers (qw_step_blocked2d.cu), built lazily
     alignas(64) unsigned char tmap[2][128];

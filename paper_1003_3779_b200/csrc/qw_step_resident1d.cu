@@ -237,6 +237,18 @@ static int launch_resident_shape(qw_sim *s, const void *in, void *out, long long
                                    : launch(step_resident1d_kernel<R, M, KIND, PHASES, false, MAXT, MINB>);
     if (rc) return rc;
     QW_LAUNCH_CHECK(s, "step_resident1d_kernel");
+    {   // site-steps actually computed: the warps the per-step cone test of the kernel leaves active
+        double touched = 0.0;
+        for (long long st = 0; st < n; ++st) {
+            if (!a.window) { touched += (double)g.en; continue; }
+            const long long r = a.radius0 + st + 1;
+            for (int wi = 0; wi < nw; ++wi) {
+                const long long lo = (long long)wi * 32 * M, hi = lo + 32 * M - 1;
+                if (lo <= a.centre + r && hi >= a.centre - r) touched += (double)((hi < g.en ? hi : g.en - 1) - lo + 1);
+            }
+        }
+        s->touched += touched * (double)g.batch;
+    }
     return QW_OK;
 }
 

@@ -89,6 +89,21 @@ static int t2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
                   : (g.boundary == QW_OPEN ? go(step_tiled2d_kernel<R, KIND, true, K>) : go(step_tiled2d_kernel<R, KIND, false, K>));
     if (rc) return rc;
     QW_LAUNCH_CHECK(s, "step_tiled2d_kernel");
+    {   // site-steps actually computed: the valid interiors of the tiles the kernel's diamond test leaves active
+        double sites = 0.0;
+        for (int tm = 0; tm < a.tiles_m; ++tm)
+            for (int tn = 0; tn < a.tiles_n; ++tn) {
+                const long long lo_m = (long long)(a.tile_m0 + tm) * TM, lo_n = (long long)(a.tile_n0 + tn) * TN;
+                if (a.dia_r >= 0) {
+                    const long long dm = a.dia_m < lo_m ? lo_m - a.dia_m : (a.dia_m > lo_m + TM - 1 ? a.dia_m - (lo_m + TM - 1) : 0);
+                    const long long dn = a.dia_n < lo_n ? lo_n - a.dia_n : (a.dia_n > lo_n + TN - 1 ? a.dia_n - (lo_n + TN - 1) : 0);
+                    if (dm + dn > a.dia_r) continue;
+                }
+                const long long hm = lo_m + TM <= g.em ? TM : g.em - lo_m, hn = lo_n + TN <= g.en ? TN : g.en - lo_n;
+                if (hm > 0 && hn > 0) sites += (double)hm * (double)hn;
+            }
+        s->touched += sites * (double)g.batch * K;
+    }
     return QW_OK;
 }
 

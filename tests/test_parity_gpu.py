@@ -573,6 +573,61 @@ def test_light_cone_diamond_of_the_tiled_kernel(qw, oracle, dev, dtype, coin):
         assert np.array_equal(got, off[0])
 
 
+def test_segment_workload_full_length_and_segment_vs_line(qw, oracle, dev):
+    """NEXT-3 (Fig. 3: "segment (left plot) ... line (right plot)"): the `seg` workload of
+    bench.py — an open Hadamard segment of 2001 sites, K0's delta start, 10 000 steps, so the front reflects off the
+    walls (PAPER.md:94-101 with RBL = 0) ten times — element by element against the oracle at its FULL length; and the
+    qualitative statement of Fig. 3: segment and line give the same distribution until the front reaches the wall and
+    different ones afterwards."""
+    import bench
+    w = bench.make_workload("seg")
+    assert w.boundary == qi.OPEN and w.sites == 2001 and w.steps == 10000
+    gpu = gpu_run(qw, w)
+    check_parity(w, gpu, oracle_run(oracle, w))
+    assert abs(gpu[2][0, 0] - 1) <= 1e-14 + 2e-16 * w.steps          # still unitary after ~10 reflections (R23 drift)
+    for steps, same in ((900, True), (1100, False)):
+        seg = qi.k0(steps=steps, half_width=1000)                    # walls at +-1000
+        line = qi.k0(steps=steps, half_width=1200)                   # walls out of reach: the paper's "line"
+        Ps = gpu_run(qw, seg)[1][0]
+        Pl = gpu_run(qw, line)[1][0][200:-200]
+        if same:
+            assert np.array_equal(Ps, Pl)
+        else:
+            assert np.max(np.abs(Ps - Pl)) > 1e-3                    # the reflected front is O(0.01) of probability
+            assert abs(Ps.sum() - 1) < 1e-12 and Pl.sum() < 1 - 1e-3  # the line has lost weight beyond +-1000
+
+
+def test_lattice_switch_in_mid_walk_drops_the_light_cone_window(qw, oracle, dev):
+    """After steps on the DIAGONAL lattice the support is a square of L1 radius 2t, larger than the diamond the tiled
+    kernel of the NATURAL lattice derives from the step count: qw_set_lattice in mid-walk must drop the window
+    (ADVICE round 1).  Delta start, 20 diagonal steps, then 24 natural steps under AUTO / TILED vs GENERIC, vs oracle."""
+    c = qi.dft4(np.complex128)
+    dc = np.array([0.5, -0.5, -0.5, 0.5], dtype=np.complex128)
+    w = qi.Workload("sw", 2, (200, 200), 1, qi.OPEN, np.dtype(np.complex128), 44, qi.COIN_UNIFORM, c, delta_site=(100, 100),
+                    delta_coin=dc, lattice=qi.DIAGONAL)
+    out = {}
+    for sched in (qw.QW_SCHED_AUTO, qw.QW_SCHED_TILED, qw.QW_SCHED_GENERIC):
+        h = qw.create_for(w)
+        try:
+            qw.load_state(h, w)
+            qw.qw_step(h, 20)
+            qw.qw_set_lattice(h, qw.QW_NATURAL)
+            assert qw.qw_get_info(h, qw.QW_INFO_WINDOW) == 0
+            qw.qw_set_schedule(h, sched, 0)
+            qw.qw_step(h, 24)
+            got = np.empty((1, w.sites, 4), dtype=w.dtype)
+            qw.qw_get_state(h, got)
+            out[sched] = got
+        finally:
+            qw.qw_destroy(h)
+    assert np.array_equal(out[qw.QW_SCHED_AUTO], out[qw.QW_SCHED_GENERIC])
+    assert np.array_equal(out[qw.QW_SCHED_TILED], out[qw.QW_SCHED_GENERIC])
+    psi = np.ascontiguousarray(w.initial_state())
+    oracle.step(w.extents, c, psi, 20, boundary=qi.OPEN, lattice=qi.DIAGONAL)
+    oracle.step(w.extents, c, psi, 24, boundary=qi.OPEN, lattice=qi.NATURAL)
+    assert np.max(np.abs(out[qw.QW_SCHED_AUTO] - psi)) <= 1e-12
+
+
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 def test_translation_covariance_bit_exact(qw, dev, dtype):
     """P12: on a periodic lattice with a uniform coin, shifting psi0 by s sites shifts psi(t) by s."""
