@@ -1,43 +1,97 @@
 // qw_reduce.cu — the per-vertex probability distribution P(x) = sum_coin |alpha|^2
 // (Figs. 3-4) and its moments (norm of PAPER.md:56 eq. 4 / :78 eq. 6; mean and
-// variance as BASELINE.json:north_star asks): per-thread FP64 accumulation, warp shuffles, a
-// shared-memory tree per block, and a second, atomic-free pass over the block partials, so the
-// result is deterministic.
+// variance as BASELINE.json:north_star asks).  Both are one streaming pass over the state planes with
+// 128-bit loads: HBM-bound.  Moments: per-thread FP64 accumulation about a LOCAL reference point, warp
+// shuffles, a shared-memory tree per block, and a second, atomic-free pass over the block partials that
+// shifts every partial to the global mean (no E[x^2] - E[x]^2 cancellation), so the result is
+// deterministic and accurate for narrow distributions far from the lattice centre.
 #include "qw_coin.cuh"
 
 namespace qw {
 
 constexpr int RED_BLOCK = 256;
 
-template <typename R, int CD>
-__global__ void __launch_bounds__(RED_BLOCK)
-prob_kernel(const typename Cx<R>::T *__restrict__ st, R *__restrict__ out, long long rows, long long em,
-            long long en, long long pitch, long long walk_stride, long long plane_stride, int chunks_per_row) {
-    const long long blk = blockIdx.x;
-    const long long rowid = blk / chunks_per_row;               // walk * em + m
-    const long long n = (blk - rowid * chunks_per_row) * RED_BLOCK + threadIdx.x;
-    if (n >= en) return;
-    const long long w = rowid / em, m = rowid - w * em;
-    const long long idx = w * walk_stride + m * pitch + n;
-    R p = 0;
+// |z|^2 summed over the CD planes for VEC consecutive sites starting at element index idx (16-byte aligned loads).
+// Accumulated in the type of the output: R for qw_probabilities, double for the moments.
+template <typename R, typename ACC, int CD, int VEC>
+__device__ __forceinline__ void site_probs(const typename Cx<R>::T *__restrict__ st, long long plane_stride, long long idx,
+                                           ACC (&p)[VEC]) {
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) p[v] = 0;
+#pragma unroll
+    for (int c = 0; c < CD; ++c) {
+        const typename Cx<R>::T *src = st + c * plane_stride + idx;
+        if constexpr (sizeof(R) == 8) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                const double2 z = __ldcs(src + v);              // streaming: every amplitude is read exactly once
+                p[v] = fma((ACC)z.x, (ACC)z.x, p[v]);
+                p[v] = fma((ACC)z.y, (ACC)z.y, p[v]);
+            }
+        } else {
+#pragma unroll
+            for (int v = 0; v < VEC; v += 2) {
+                const float4 z = __ldcs(reinterpret_cast<const float4 *>(src + v));
+                p[v] = fma((ACC)z.x, (ACC)z.x, p[v]);
+                p[v] = fma((ACC)z.y, (ACC)z.y, p[v]);
+                p[v + 1] = fma((ACC)z.z, (ACC)z.z, p[v + 1]);
+                p[v + 1] = fma((ACC)z.w, (ACC)z.w, p[v + 1]);
+            }
+        }
+    }
+}
+template <typename R, typename ACC, int CD>
+__device__ __forceinline__ ACC site_prob1(const typename Cx<R>::T *__restrict__ st, long long plane_stride, long long idx) {
+    ACC p = 0;
 #pragma unroll
     for (int c = 0; c < CD; ++c) {
         const typename Cx<R>::T z = st[c * plane_stride + idx];
-        p = fma_rn(z.x, z.x, p);
-        p = fma_rn(z.y, z.y, p);
+        p = fma((ACC)z.x, (ACC)z.x, p);
+        p = fma((ACC)z.y, (ACC)z.y, p);
     }
-    out[rowid * en + n] = p;
+    return p;
+}
+
+// sites per thread: two 16-byte loads per plane in flight (complex128: 2 sites, complex64: 4 sites)
+template <typename R> struct RedVec { static constexpr int value = sizeof(R) == 8 ? 2 : 4; };
+
+template <typename R, int CD>
+__global__ void __launch_bounds__(RED_BLOCK)
+prob_kernel(const typename Cx<R>::T *__restrict__ st, R *__restrict__ out, long long em, long long en, long long pitch,
+            long long walk_stride, long long plane_stride, int chunks_per_row) {
+    constexpr int VEC = RedVec<R>::value;
+    const long long blk = blockIdx.x;
+    const long long rowid = blk / chunks_per_row;               // walk * em + m
+    const long long n = ((blk - rowid * chunks_per_row) * RED_BLOCK + threadIdx.x) * VEC;
+    if (n >= en) return;
+    const long long w = rowid / em, m = rowid - w * em;
+    const long long idx = w * walk_stride + m * pitch + n;
+    R *o = out + rowid * en + n;
+    if (n + VEC <= en) {
+        R p[VEC];
+        site_probs<R, R, CD, VEC>(st, plane_stride, idx, p);
+        if ((reinterpret_cast<uintptr_t>(o) & 15) == 0) {       // rows of odd length: not every row start is 16-byte aligned
+            if constexpr (sizeof(R) == 8) *reinterpret_cast<double2 *>(o) = make_double2(p[0], p[1]);
+            else *reinterpret_cast<float4 *>(o) = make_float4(p[0], p[1], p[2], p[3]);
+        } else {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) o[v] = p[v];
+        }
+    } else {
+        for (int v = 0; n + v < en; ++v) o[v] = site_prob1<R, R, CD>(st, plane_stride, idx + v);
+    }
 }
 
 template <typename R, int CD>
 static int launch_prob_t(qw_sim *s, const void *state, void *out) {
     const Geom &g = s->g;
-    const int cpr = (int)((g.en + RED_BLOCK - 1) / RED_BLOCK);
+    constexpr int PER_BLOCK = RED_BLOCK * RedVec<R>::value;
+    const int cpr = (int)((g.en + PER_BLOCK - 1) / PER_BLOCK);
     const long long blocks = g.batch * g.em * cpr;
     if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
     prob_kernel<R, CD><<<(unsigned)blocks, RED_BLOCK, 0, s->stream>>>(
-        static_cast<const typename Cx<R>::T *>(state), static_cast<R *>(out), g.batch * g.em, g.em, g.en,
-        g.pitch, g.walk_stride, g.plane_stride, cpr);
+        static_cast<const typename Cx<R>::T *>(state), static_cast<R *>(out), g.em, g.en, g.pitch, g.walk_stride,
+        g.plane_stride, cpr);
     QW_LAUNCH_CHECK(s, "prob_kernel");
     return QW_OK;
 }
@@ -49,8 +103,9 @@ int launch_probabilities(qw_sim *s, const void *state, void *out) {
 }
 
 // ---- moments -----------------------------------------------------------------------------------
-// Raw sums per walk: S0 = sum P, Sm = sum xm P, Sn = sum xn P, Smm, Snn, Smn  (1D uses S0, Sn, Snn).
-constexpr int NMOM = 6;
+// Block partials, per (walk, block): the reference point (rm, rn) in lattice-centred coordinates and the raw sums ABOUT it:
+// S0 = sum P, Sm = sum (xm - rm) P, Sn = sum (xn - rn) P, Smm, Snn, Smn.
+constexpr int NPART = 8;
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -58,112 +113,149 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
+// A block owns a CONTIGUOUS range of work items; an item is one chunk of RED_BLOCK * VEC sites of one lattice row.
+// Row and chunk come from one division per ITEM (not per site); inside an item every thread takes VEC consecutive sites.
 template <typename R, int CD>
 __global__ void __launch_bounds__(RED_BLOCK)
-moments_partial_kernel(const typename Cx<R>::T *__restrict__ st, double *__restrict__ partials, long long em,
-                       long long en, long long pitch, long long walk_stride, long long plane_stride,
-                       int blocks_per_walk) {
-    const long long w = blockIdx.y;
+moments_partial_kernel(const typename Cx<R>::T *__restrict__ st, double *__restrict__ partials, long long em, long long en,
+                       long long pitch, long long walk_stride, long long plane_stride, int blocks_per_walk,
+                       long long items_per_block, int chunks_per_row) {
+    constexpr int VEC = RedVec<R>::value;
+    const long long w = blockIdx.x / blocks_per_walk;
+    const int b = (int)(blockIdx.x - w * blocks_per_walk);
+    const long long items = em * chunks_per_row;
+    const long long it0 = (long long)b * items_per_block;
+    const long long it1 = it0 + items_per_block < items ? it0 + items_per_block : items;
     const long long cm = em / 2, cn = en / 2;
-    const long long sites = em * en;
-    double acc[NMOM] = {0, 0, 0, 0, 0, 0};
-    for (long long x = (long long)blockIdx.x * RED_BLOCK + threadIdx.x; x < sites;
-         x += (long long)blocks_per_walk * RED_BLOCK) {
-        const long long m = x / en, n = x - m * en;
+    // reference point of the block: its first site
+    const long long m_ref = it0 / chunks_per_row, n_ref = (it0 - m_ref * chunks_per_row) * (RED_BLOCK * VEC);
+    double a0 = 0, am = 0, an = 0, amm = 0, ann = 0, amn = 0;
+#pragma unroll 2
+    for (long long it = it0; it < it1; ++it) {
+        const long long m = it / chunks_per_row;
+        const long long n = ((it - m * chunks_per_row) * RED_BLOCK + threadIdx.x) * VEC;
+        if (n >= en) continue;
         const long long idx = w * walk_stride + m * pitch + n;
-        double p = 0.0;
+        double p[VEC];
+        int nv = VEC;
+        if (n + VEC <= en) {
+            site_probs<R, double, CD, VEC>(st, plane_stride, idx, p);
+        } else {
+            nv = (int)(en - n);
 #pragma unroll
-        for (int c = 0; c < CD; ++c) {
-            const typename Cx<R>::T z = st[c * plane_stride + idx];
-            const double re = (double)z.x, im = (double)z.y;
-            p = fma(re, re, p);
-            p = fma(im, im, p);
+            for (int v = 0; v < VEC; ++v) p[v] = v < nv ? site_prob1<R, double, CD>(st, plane_stride, idx + v) : 0.0;
         }
-        const double xm = (double)(m - cm), xn = (double)(n - cn);
-        acc[0] += p;
-        acc[1] += xm * p;
-        acc[2] += xn * p;
-        acc[3] += xm * xm * p;
-        acc[4] += xn * xn * p;
-        acc[5] += xm * xn * p;
-    }
-    __shared__ double sm[NMOM][RED_BLOCK / 32];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+        const double dm = (double)(m - m_ref), dn0 = (double)(n - n_ref);
+        double s0 = 0, s1 = 0, s2 = 0;
 #pragma unroll
-    for (int k = 0; k < NMOM; ++k) {
+        for (int v = 0; v < VEC; ++v) {
+            const double dn = dn0 + v;
+            s0 += p[v];
+            s1 = fma(dn, p[v], s1);
+            s2 = fma(dn * dn, p[v], s2);
+        }
+        a0 += s0; an += s1; ann += s2;
+        am = fma(dm, s0, am); amm = fma(dm * dm, s0, amm); amn = fma(dm, s1, amn);
+    }
+    __shared__ double sm[6][RED_BLOCK / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    double acc[6] = {a0, am, an, amm, ann, amn};
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
         const double v = warp_sum(acc[k]);
         if (lane == 0) sm[k][wid] = v;
     }
     __syncthreads();
     if (wid == 0) {
+        double *out = partials + (size_t)blockIdx.x * NPART;
 #pragma unroll
-        for (int k = 0; k < NMOM; ++k) {
+        for (int k = 0; k < 6; ++k) {
             double v = (lane < RED_BLOCK / 32) ? sm[k][lane] : 0.0;
             v = warp_sum(v);
-            if (lane == 0) partials[(w * blocks_per_walk + blockIdx.x) * NMOM + k] = v;
+            if (lane == 0) out[2 + k] = v;
         }
+        if (lane == 0) { out[0] = (double)(m_ref - cm); out[1] = (double)(n_ref - cn); }
     }
 }
 
-// One warp per walk folds the block partials in a fixed order and forms the normalised moments.
+// One warp per walk: pass 1 folds the block partials (fixed order) into the norm and the means, pass 2 shifts every
+// partial to the mean and folds the central second moments.  A walk whose norm is exactly 0 reports all zeros.
 __global__ void moments_final_kernel(const double *__restrict__ partials, double *__restrict__ out,
                                      long long batch, int blocks_per_walk, int dim) {
     const long long w = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (w >= batch) return;
-    double acc[NMOM] = {0, 0, 0, 0, 0, 0};
-    for (int b = lane; b < blocks_per_walk; b += 32)
-#pragma unroll
-        for (int k = 0; k < NMOM; ++k) acc[k] += partials[(w * blocks_per_walk + b) * NMOM + k];
-#pragma unroll
-    for (int k = 0; k < NMOM; ++k) acc[k] = warp_sum(acc[k]);
+    const double *P = partials + (size_t)w * blocks_per_walk * NPART;
+    double s0 = 0, sm = 0, sn = 0;
+    for (int b = lane; b < blocks_per_walk; b += 32) {
+        const double *q = P + (size_t)b * NPART;
+        s0 += q[2];
+        sm += fma(q[0], q[2], q[3]);
+        sn += fma(q[1], q[2], q[4]);
+    }
+    s0 = warp_sum(s0); sm = warp_sum(sm); sn = warp_sum(sn);
+    const bool empty = !(s0 != 0.0);
+    const double mm = empty ? 0.0 : sm / s0, mn = empty ? 0.0 : sn / s0;
+    double cmm = 0, cnn = 0, cmn = 0;
+    for (int b = lane; b < blocks_per_walk; b += 32) {
+        const double *q = P + (size_t)b * NPART;
+        const double dm = q[0] - mm, dn = q[1] - mn;          // block reference relative to the mean
+        cmm += q[5] + 2.0 * dm * q[3] + dm * dm * q[2];
+        cnn += q[6] + 2.0 * dn * q[4] + dn * dn * q[2];
+        cmn += q[7] + dm * q[4] + dn * q[3] + dm * dn * q[2];
+    }
+    cmm = warp_sum(cmm); cnn = warp_sum(cnn); cmn = warp_sum(cmn);
     if (lane == 0) {
-        const double s0 = acc[0];
-        const double mm = acc[1] / s0, mn = acc[2] / s0;
+        const double inv = empty ? 0.0 : 1.0 / s0;
         if (dim == 1) {
             out[w * 3 + 0] = s0;
             out[w * 3 + 1] = mn;
-            out[w * 3 + 2] = acc[4] / s0 - mn * mn;
+            out[w * 3 + 2] = cnn * inv;
         } else {
             out[w * 6 + 0] = s0;
             out[w * 6 + 1] = mm;
             out[w * 6 + 2] = mn;
-            out[w * 6 + 3] = acc[3] / s0 - mm * mm;
-            out[w * 6 + 4] = acc[4] / s0 - mn * mn;
-            out[w * 6 + 5] = acc[5] / s0 - mm * mn;
+            out[w * 6 + 3] = cmm * inv;
+            out[w * 6 + 4] = cnn * inv;
+            out[w * 6 + 5] = cmn * inv;
         }
     }
 }
 
+template <typename R, int CD>
+static void launch_mom_t(qw_sim *s, const void *state, unsigned grid, int bpw, long long ipb, int cpr) {
+    const Geom &g = s->g;
+    moments_partial_kernel<R, CD><<<grid, RED_BLOCK, 0, s->stream>>>(
+        static_cast<const typename Cx<R>::T *>(state), s->partials, g.em, g.en, g.pitch, g.walk_stride, g.plane_stride, bpw,
+        ipb, cpr);
+}
+
 int launch_moments(qw_sim *s, const void *state, double *out) {
     const Geom &g = s->g;
-    // enough blocks to fill the machine, never more than the work
-    long long want = (g.sites + (long long)RED_BLOCK * 8 - 1) / ((long long)RED_BLOCK * 8);
-    long long cap = (long long)s->sm_count * 8 / (g.batch < 1 ? 1 : g.batch);
-    if (cap < 1) cap = 1;
-    if (want > cap) want = cap;
-    if (want < 1) want = 1;
-    const int bpw = (int)want;
-    if (g.batch > 65535) return fail(QW_EUNSUPPORTED, "batch larger than 65535 walks");
-    const size_t need = (size_t)g.batch * bpw * NMOM;
+    const int vec = s->dtype == QW_C128 ? RedVec<double>::value : RedVec<float>::value;
+    const int cpr = (int)((g.en + (long long)RED_BLOCK * vec - 1) / ((long long)RED_BLOCK * vec));
+    const long long items = g.em * cpr;
+    // enough blocks to fill the machine (16 CTAs of 256 threads per SM and a few waves), never more than the work
+    long long bpw = (long long)s->sm_count * 32 / g.batch;
+    if (bpw < 1) bpw = 1;
+    if (bpw > items) bpw = items;
+    const long long ipb = (items + bpw - 1) / bpw;
+    bpw = (items + ipb - 1) / ipb;
+    const long long blocks = bpw * g.batch;
+    if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "batch too large for one launch");
+    const size_t need = (size_t)blocks * NPART;
     if (need > s->partials_count) {
-        if (s->partials) cudaFree(s->partials);
+        if (s->partials) { cudaStreamSynchronize(s->stream); cudaFree(s->partials); }
         s->partials = nullptr; s->partials_count = 0;
         QW_CUDA(cudaMalloc(&s->partials, need * sizeof(double)));
         s->partials_count = need;
     }
-    dim3 grid((unsigned)bpw, (unsigned)g.batch);
-#define QW_MOM(R, CD)                                                                                   \
-    moments_partial_kernel<R, CD><<<grid, RED_BLOCK, 0, s->stream>>>(                                   \
-        static_cast<const Cx<R>::T *>(state), s->partials, g.em, g.en, g.pitch, g.walk_stride,          \
-        g.plane_stride, bpw)
-    if (s->dtype == QW_C128) { if (g.cdim == 2) QW_MOM(double, 2); else QW_MOM(double, 4); }
-    else                     { if (g.cdim == 2) QW_MOM(float, 2);  else QW_MOM(float, 4); }
-#undef QW_MOM
+    if (s->dtype == QW_C128) { if (g.cdim == 2) launch_mom_t<double, 2>(s, state, (unsigned)blocks, (int)bpw, ipb, cpr); else launch_mom_t<double, 4>(s, state, (unsigned)blocks, (int)bpw, ipb, cpr); }
+    else                     { if (g.cdim == 2) launch_mom_t<float, 2>(s, state, (unsigned)blocks, (int)bpw, ipb, cpr);  else launch_mom_t<float, 4>(s, state, (unsigned)blocks, (int)bpw, ipb, cpr); }
     QW_LAUNCH_CHECK(s, "moments_partial_kernel");
     const int warps = 4;
     moments_final_kernel<<<(unsigned)((g.batch + warps - 1) / warps), warps * 32, 0, s->stream>>>(
-        s->partials, out, g.batch, bpw, g.dim);
+        s->partials, out, g.batch, (int)bpw, g.dim);
     QW_LAUNCH_CHECK(s, "moments_final_kernel");
     return QW_OK;
 }
