@@ -40,6 +40,66 @@ static int ensure_scratch(qw_sim *s, size_t bytes) {
     return QW_OK;
 }
 
+constexpr size_t QW_STAGE_BYTES = 64u << 20;
+
+static int ensure_stage(qw_sim *s) {
+    if (s->stage_ready) return QW_OK;
+    for (int i = 0; i < 2; ++i) {
+        if (cudaMalloc(&s->stage[i], QW_STAGE_BYTES) != cudaSuccess) {
+            cudaGetLastError();
+            if (i == 1) { cudaFree(s->stage[0]); s->stage[0] = nullptr; }
+            return fail(QW_ENOMEM, "cannot allocate the %zu-byte staging buffers", QW_STAGE_BYTES);
+        }
+    }
+    QW_CUDA(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+        QW_CUDA(cudaEventCreateWithFlags(&s->ev_copy[i], cudaEventDisableTiming));
+        QW_CUDA(cudaEventCreateWithFlags(&s->ev_kernel[i], cudaEventDisableTiming));
+    }
+    s->stage_ready = true;
+    return QW_OK;
+}
+
+// Host AoS amplitudes <-> device SoA planes in chunks: copy stream and handle stream alternate over two staging buffers.
+static int stream_state(qw_sim *s, void *host, bool to_device) {
+    int rc = ensure_stage(s);
+    if (rc) return rc;
+    const Geom &g = s->g;
+    const size_t site_bytes = (size_t)g.cdim * s->esize;
+    const long long total = g.batch * g.sites;
+    const long long per_chunk = (long long)(QW_STAGE_BYTES / site_bytes);
+    // the copy stream must not run ahead of work already queued on the handle's stream (and vice versa)
+    QW_CUDA(cudaEventRecord(s->ev_kernel[0], s->stream));
+    QW_CUDA(cudaStreamWaitEvent(s->copy_stream, s->ev_kernel[0], 0));
+    QW_CUDA(cudaEventRecord(s->ev_kernel[1], s->stream));
+    int c = 0;
+    for (long long first = 0; first < total; first += per_chunk, ++c) {
+        const int b = c & 1;
+        const long long count = total - first < per_chunk ? total - first : per_chunk;
+        char *h = static_cast<char *>(host) + (size_t)first * site_bytes;
+        if (to_device) {
+            QW_CUDA(cudaStreamWaitEvent(s->copy_stream, s->ev_kernel[b], 0));       // buffer b consumed by chunk c-2
+            QW_CUDA(cudaMemcpyAsync(s->stage[b], h, (size_t)count * site_bytes, cudaMemcpyHostToDevice, s->copy_stream));
+            QW_CUDA(cudaEventRecord(s->ev_copy[b], s->copy_stream));
+            QW_CUDA(cudaStreamWaitEvent(s->stream, s->ev_copy[b], 0));
+            rc = launch_aos_to_soa(s, s->stage[b], state_ptr(s, s->cur), first, count);
+            if (rc) return rc;
+            QW_CUDA(cudaEventRecord(s->ev_kernel[b], s->stream));
+        } else {
+            QW_CUDA(cudaStreamWaitEvent(s->stream, s->ev_copy[b], 0));              // buffer b copied out by chunk c-2
+            rc = launch_soa_to_aos(s, state_ptr(s, s->cur), s->stage[b], first, count);
+            if (rc) return rc;
+            QW_CUDA(cudaEventRecord(s->ev_kernel[b], s->stream));
+            QW_CUDA(cudaStreamWaitEvent(s->copy_stream, s->ev_kernel[b], 0));
+            QW_CUDA(cudaMemcpyAsync(h, s->stage[b], (size_t)count * site_bytes, cudaMemcpyDeviceToHost, s->copy_stream));
+            QW_CUDA(cudaEventRecord(s->ev_copy[b], s->copy_stream));
+        }
+    }
+    QW_CUDA(cudaStreamSynchronize(s->copy_stream));        // the host buffer is reusable / filled on return
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    return QW_OK;
+}
+
 static int classify_coin(const double *C, int cdim, int dtype) {
     auto re = [&](int a, int b) { return C[2 * (a * cdim + b)]; };
     auto im = [&](int a, int b) { return C[2 * (a * cdim + b) + 1]; };
@@ -186,6 +246,11 @@ int qw_destroy(qw_sim *s) {
     if (s->d_broken) cudaFree(s->d_broken);
     if (s->scratch) cudaFree(s->scratch);
     if (s->partials) cudaFree(s->partials);
+    if (s->stage_ready) {
+        cudaStreamSynchronize(s->copy_stream);
+        for (int i = 0; i < 2; ++i) { cudaFree(s->stage[i]); cudaEventDestroy(s->ev_copy[i]); cudaEventDestroy(s->ev_kernel[i]); }
+        cudaStreamDestroy(s->copy_stream);
+    }
     cudaGetLastError();
     delete s;
     return QW_OK;
@@ -298,18 +363,12 @@ int qw_set_state(qw_sim *s, const void *amps) {
     if (!amps) return fail(QW_EINVAL, "amps is NULL");
     const Geom &g = s->g;
     const size_t bytes = (size_t)g.batch * (size_t)g.sites * (size_t)g.cdim * s->esize;
-    const void *src = amps;
-    if (!is_device_ptr(amps)) {
-        int rc = ensure_scratch(s, bytes);
-        if (rc) return rc;
-        QW_CUDA(cudaMemcpyAsync(s->scratch, amps, bytes, cudaMemcpyHostToDevice, s->stream));
-        src = s->scratch;
-    }
+    (void)bytes;
     s->cur = 0;
     if (g.pitch != g.en || g.ghost) QW_CUDA(cudaMemsetAsync(s->buf[0], 0, s->state_bytes, s->stream));
-    int rc = launch_aos_to_soa(s, src, state_ptr(s, 0));
+    int rc = is_device_ptr(amps) ? launch_aos_to_soa(s, amps, state_ptr(s, 0))
+                                 : stream_state(s, const_cast<void *>(amps), true);   // chunked; host buffer reusable on return
     if (rc) return rc;
-    if (src == s->scratch) QW_CUDA(cudaStreamSynchronize(s->stream));   // host buffer reusable on return
     s->has_state = true; s->t = 0; s->window_valid = false;
     return QW_OK;
 }
@@ -355,14 +414,9 @@ int qw_get_state(const qw_sim *cs, void *amps) {
     if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
     const Geom &g = s->g;
     const size_t bytes = (size_t)g.batch * (size_t)g.sites * (size_t)g.cdim * s->esize;
+    (void)bytes;
     if (is_device_ptr(amps)) return launch_soa_to_aos(s, state_ptr(s, s->cur), amps);
-    int rc = ensure_scratch(s, bytes);
-    if (rc) return rc;
-    rc = launch_soa_to_aos(s, state_ptr(s, s->cur), s->scratch);
-    if (rc) return rc;
-    QW_CUDA(cudaMemcpyAsync(amps, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
-    QW_CUDA(cudaStreamSynchronize(s->stream));
-    return QW_OK;
+    return stream_state(s, amps, false);
 }
 
 int qw_step(qw_sim *s, int64_t n) {

@@ -97,8 +97,16 @@ struct qw_sim {
     alignas(64) unsigned char tmap_t[2][128];   // ... of the register-tiled kernel (qw_step_tiled2d.cuh)
     bool tmap_t_ready;
 
+    // host <-> device streaming of the state (qw_set_state / qw_get_state with host buffers): two staging buffers of
+    // QW_STAGE_BYTES on the device, a private copy stream and events, so the PCIe copy of chunk i+1 overlaps the layout
+    // kernel of chunk i and no state-sized scratch is needed
+    void *stage[2];
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_copy[2], ev_kernel[2];
+    bool stage_ready;
+
     // scratch
-    void *scratch;           // staging for host <-> device transposes and outputs
+    void *scratch;           // staging for outputs to host buffers (probabilities, moments)
     size_t scratch_bytes;
     double *partials;        // moment partial sums
     size_t partials_count;
@@ -133,8 +141,8 @@ void clear_error();
 
 // ---- kernels' host-side launchers (one per translation unit) -------------------------------
 // qw_layout.cu
-int launch_aos_to_soa(qw_sim *s, const void *aos_dev, void *soa);
-int launch_soa_to_aos(qw_sim *s, const void *soa, void *aos_dev);
+int launch_aos_to_soa(qw_sim *s, const void *aos_dev, void *soa, long long first = 0, long long count = -1);
+int launch_soa_to_aos(qw_sim *s, const void *soa, void *aos_dev, long long first = 0, long long count = -1);
 int launch_delta(qw_sim *s, const long long *site, const double *coin_vec);
 
 // qw_step.cu : one launch per step, scatter form.  fast = uniform coin, no phases, no links, natural.

@@ -10,48 +10,53 @@ constexpr int LAYOUT_BLOCK = 256;
 template <typename R, int CD, bool TO_SOA>
 __global__ void __launch_bounds__(LAYOUT_BLOCK)
 transpose_kernel(const typename Cx<R>::T *__restrict__ src, typename Cx<R>::T *__restrict__ dst,
-                 long long total_sites, long long sites, long long en, long long pitch,
+                 long long first, long long count, long long sites, long long en, long long pitch,
                  long long walk_stride, long long plane_stride) {
-    const long long i = (long long)blockIdx.x * LAYOUT_BLOCK + threadIdx.x;   // walk * sites + site
-    if (i >= total_sites) return;
+    // the AoS side holds the flat sites [first, first + count) (flat = walk * sites + site), starting at its element 0
+    const long long j = (long long)blockIdx.x * LAYOUT_BLOCK + threadIdx.x;
+    if (j >= count) return;
+    const long long i = first + j;
     const long long w = i / sites, x = i - w * sites;
     const long long m = x / en, n = x - m * en;
     const long long idx = w * walk_stride + m * pitch + n;
 #pragma unroll
     for (int c = 0; c < CD; ++c) {
-        if (TO_SOA) dst[c * plane_stride + idx] = src[i * CD + c];
-        else        dst[i * CD + c] = src[c * plane_stride + idx];
+        if (TO_SOA) dst[c * plane_stride + idx] = src[j * CD + c];
+        else        dst[j * CD + c] = src[c * plane_stride + idx];
     }
 }
 
 template <typename R, int CD, bool TO_SOA>
-static int launch_transpose_t(qw_sim *s, const void *src, void *dst) {
+static int launch_transpose_t(qw_sim *s, const void *src, void *dst, long long first, long long count) {
     typedef typename Cx<R>::T V;
     const Geom &g = s->g;
-    const long long total = g.batch * g.sites;
-    const long long blocks = (total + LAYOUT_BLOCK - 1) / LAYOUT_BLOCK;
+    const long long blocks = (count + LAYOUT_BLOCK - 1) / LAYOUT_BLOCK;
+    if (blocks <= 0) return QW_OK;
     if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
     transpose_kernel<R, CD, TO_SOA><<<(unsigned)blocks, LAYOUT_BLOCK, 0, s->stream>>>(
-        static_cast<const V *>(src), static_cast<V *>(dst), total, g.sites, g.en, g.pitch,
+        static_cast<const V *>(src), static_cast<V *>(dst), first, count, g.sites, g.en, g.pitch,
         g.walk_stride, g.plane_stride);
     QW_LAUNCH_CHECK(s, "transpose_kernel");
     return QW_OK;
 }
 
-int launch_aos_to_soa(qw_sim *s, const void *aos, void *soa) {
+// `aos` points at the amplitudes of flat site `first`; count < 0 = all sites of all walks
+int launch_aos_to_soa(qw_sim *s, const void *aos, void *soa, long long first, long long count) {
+    if (count < 0) count = s->g.batch * s->g.sites - first;
     if (s->dtype == QW_C128)
-        return s->g.cdim == 2 ? launch_transpose_t<double, 2, true>(s, aos, soa)
-                              : launch_transpose_t<double, 4, true>(s, aos, soa);
-    return s->g.cdim == 2 ? launch_transpose_t<float, 2, true>(s, aos, soa)
-                          : launch_transpose_t<float, 4, true>(s, aos, soa);
+        return s->g.cdim == 2 ? launch_transpose_t<double, 2, true>(s, aos, soa, first, count)
+                              : launch_transpose_t<double, 4, true>(s, aos, soa, first, count);
+    return s->g.cdim == 2 ? launch_transpose_t<float, 2, true>(s, aos, soa, first, count)
+                          : launch_transpose_t<float, 4, true>(s, aos, soa, first, count);
 }
 
-int launch_soa_to_aos(qw_sim *s, const void *soa, void *aos) {
+int launch_soa_to_aos(qw_sim *s, const void *soa, void *aos, long long first, long long count) {
+    if (count < 0) count = s->g.batch * s->g.sites - first;
     if (s->dtype == QW_C128)
-        return s->g.cdim == 2 ? launch_transpose_t<double, 2, false>(s, soa, aos)
-                              : launch_transpose_t<double, 4, false>(s, soa, aos);
-    return s->g.cdim == 2 ? launch_transpose_t<float, 2, false>(s, soa, aos)
-                          : launch_transpose_t<float, 4, false>(s, soa, aos);
+        return s->g.cdim == 2 ? launch_transpose_t<double, 2, false>(s, soa, aos, first, count)
+                              : launch_transpose_t<double, 4, false>(s, soa, aos, first, count);
+    return s->g.cdim == 2 ? launch_transpose_t<float, 2, false>(s, soa, aos, first, count)
+                          : launch_transpose_t<float, 4, false>(s, soa, aos, first, count);
 }
 
 template <typename R>

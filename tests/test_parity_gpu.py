@@ -739,8 +739,10 @@ def test_error_codes_on_device(qw, dev):
 
 
 def test_set_state_round_trip_is_exact(qw, dev):
+    """Host buffers stream through two 64 MiB staging buffers (copy of chunk i+1 under the layout kernel of chunk i):
+    the last two cases span several chunks with a ragged last one, and chunk borders inside a walk and inside a row."""
     for dtype in (np.complex128, np.complex64):
-        for ext, batch in (((1001,), 3), ((33, 47), 2)):
+        for ext, batch in (((1001,), 3), ((33, 47), 2), ((3000001,), 2), ((1500, 1401), 1)):
             sites = int(np.prod(ext))
             st = qi.random_state(5, batch, sites, 2 * len(ext), dtype)
             h = qw.qw_create_batch(batch, len(ext), ext, 2 * len(ext), qw.dtype_code(dtype), qw.QW_PERIODIC)
