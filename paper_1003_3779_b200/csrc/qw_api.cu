@@ -430,7 +430,8 @@ int qw_step(qw_sim *s, int64_t n) {
     int sched = s->sched;
     if (sched == QW_SCHED_AUTO)
         sched = resident1d_eligible(s) ? QW_SCHED_RESIDENT
-              : (blocked1d_eligible(s) && n >= 4) ? QW_SCHED_BLOCKED
+              : ((blocked1d_eligible(s) && n >= 4) ||
+                 (chain1d_eligible(s, chain1d_granule(s)) && n >= chain1d_granule(s))) ? QW_SCHED_BLOCKED
               : (tiled2d_eligible(s) && n >= 2) ? QW_SCHED_TILED : QW_SCHED_FUSED;
     if (sched == QW_SCHED_RESIDENT) {
         if (!resident1d_eligible(s))
@@ -441,7 +442,7 @@ int qw_step(qw_sim *s, int64_t n) {
         s->last_sched = sched; s->last_k = (int)(n > 0x7fffffff ? 0x7fffffff : n);
         return QW_OK;
     }
-    if (sched == QW_SCHED_BLOCKED && !blocked1d_eligible(s) && !blocked2d_eligible(s))
+    if (sched == QW_SCHED_BLOCKED && !blocked1d_eligible(s) && !blocked2d_eligible(s) && !chain1d_eligible(s, chain1d_granule(s)))
         return fail(QW_EUNSUPPORTED, "the temporally blocked schedule needs a uniform coin without phases or link mask on a 1D "
                                      "lattice of >= %d sites or a natural 2D lattice of >= 32 x 32 sites",
                     32 * blocked1d_granule(s));
@@ -498,12 +499,13 @@ int qw_step(qw_sim *s, int64_t n) {
         if (kchain > chain1d_max_k(s)) kchain = chain1d_max_k(s);
         kchain = kchain / M * M;
         bool chain = kchain >= M && chain1d_eligible(s, kchain);
-        if (chain && s->blocked1d_kernel == 0) chain = chain1d_cost(s, kchain) / kchain < blocked1d_cost(s, kmax) / kmax;
-        if (s->blocked1d_kernel == 1) chain = false;
+        const bool halo = blocked1d_eligible(s);       // no random broken links in the halo kernel
+        if (chain && halo && s->blocked1d_kernel == 0) chain = chain1d_cost(s, kchain) / kchain < blocked1d_cost(s, kmax) / kmax;
+        if (halo && s->blocked1d_kernel == 1) chain = false;
         s->last_k = chain ? kchain : kmax;
         // multiples of M with the big tiles, then a remainder of 4 .. 15 steps with short 8- / 4-step launches (small
         // tiles, the fused kernel's arithmetic), then at most 3 fused single steps
-        while (remaining >= 4) {
+        while (remaining >= (halo ? 4 : M)) {
             int rc;
             int kk;
             if (chain && remaining >= M) {

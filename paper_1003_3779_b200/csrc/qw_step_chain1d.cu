@@ -24,6 +24,7 @@
 //
 // HBM bytes per site-step: coin_dim*sizeof(complex) * (2 + 1/tiles_per_chain) / k.
 #include "qw_coin.cuh"
+#include "qw_philox.cuh"
 
 namespace qw {
 
@@ -39,6 +40,17 @@ struct Chain1dArgs {
     int k;                   // steps in this launch: a multiple of M, <= 16*M
     R coin[8];
     R scale_m;               // deferred-scale Hadamard: s^M, applied once per M steps
+    // random broken links redrawn every step (qw_set_random_broken_links; RBL template instances only)
+    unsigned rbl_key0, rbl_key1;
+    unsigned long long rbl_thr;     // floor(p * 2^32)
+    unsigned t0;                    // step index of the first step of this launch (low 32 bits)
+};
+
+// What the RBL instances carry through the steps: the lattice coordinate of the lane's logical site 0 and the counter words.
+struct Chain1dLinks {
+    long long x0, n_sites;          // site of logical 0 of this lane at the current step (0 <= x0 < N); ring length
+    unsigned t, walk, key0, key1;
+    unsigned long long thr;
 };
 
 // ---- exchange by warp shuffles (complex64) -------------------------------------------------------------------------
@@ -84,9 +96,16 @@ template <typename R> struct Chain1dExchange {
 };
 
 // One walk step, U = step index inside the M-step period.
-template <typename R, int M, int KIND, int U>
+//
+// RBL (random broken links, eqs. 9-10): the link between the sites at logical positions Q and Q + 1
+// carries phi_R[Q] to the right and phi_L[Q + 1] to the left; broken, both stay where they are with the opposite coin,
+// i.e. the pair (R'[Q], L'[Q - 1]) = (phi_R[Q], phi_L[Q + 1]) is SWAPPED.  In this frame both members of the pair sit in
+// the same lane — Rp[q] and the register that holds phi_L[q + 1] (for q = M - 1: the one just received from the lane
+// above) — so a broken link is a predicated swap of two registers; its state is one Philox call per (site, step).
+template <typename R, int M, int KIND, bool RBL, int U>
 __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
-                                             typename Cx<R>::T *&wptr, const typename Cx<R>::T *&rptr, int winc, int rinc) {
+                                             typename Cx<R>::T *&wptr, const typename Cx<R>::T *&rptr, int winc, int rinc,
+                                             Chain1dLinks &lk) {
     typedef typename Cx<R>::T V;
     typedef Chain1dExchange<R> EX;
 #pragma unroll
@@ -108,8 +127,25 @@ __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M],
         Rp[q] = v[0];
         Lp[p] = v[1];
     }
-    // phi_L of logical sites 0 and 1 leaves the lane: it becomes L' of logical sites M-2, M-1 of the lane below
     constexpr int P0 = (2 * U) % M, P1 = (2 * U + 1) % M;
+    [[maybe_unused]] auto link_broken = [&](int q) -> bool {      // link owned by the site at logical position q
+        long long x = lk.x0 + q;
+        if (x >= lk.n_sites) x -= lk.n_sites;
+        const unsigned word = philox4x32_10_word((unsigned)x, (unsigned)((unsigned long long)x >> 32), lk.t, lk.walk,
+                                                 lk.key0, lk.key1, 0);
+        return (unsigned long long)word < lk.thr;
+    };
+    if constexpr (RBL) {
+#pragma unroll
+        for (int q = 0; q + 1 < M; ++q) {
+            if (link_broken(q)) {
+                const cplx<R> tmp = Rp[q];
+                Rp[q] = Lp[(q + 1 + 2 * U) % M];
+                Lp[(q + 1 + 2 * U) % M] = tmp;
+            }
+        }
+    }
+    // phi_L of logical sites 0 and 1 leaves the lane: it becomes L' of logical sites M-2, M-1 of the lane below
     V z0, z1;
     z0.x = Lp[P0].re; z0.y = Lp[P0].im; z1.x = Lp[P1].re; z1.y = Lp[P1].im;
     if constexpr (EX::SMEM) {
@@ -130,14 +166,24 @@ __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M],
         Lp[P0] = chain_shfl_from(o0, rinc >> 8);
         Lp[P1] = chain_shfl_from(o1, rinc >> 8);
     }
+    if constexpr (RBL) {
+        if (link_broken(M - 1)) {                                  // partner: what the lane above just handed over
+            const cplx<R> tmp = Rp[M - 1];
+            Rp[M - 1] = Lp[P0];
+            Lp[P0] = tmp;
+        }
+        lk.t += 1;                                                 // next step: the frame has moved one site to the right
+        lk.x0 = lk.x0 + 1 == lk.n_sites ? 0 : lk.x0 + 1;
+    }
 }
 
-template <typename R, int M, int KIND, int U>
+template <typename R, int M, int KIND, bool RBL, int U>
 struct Chain1dUnroll {
     static __device__ __forceinline__ void run(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
-                                               typename Cx<R>::T *&wptr, const typename Cx<R>::T *&rptr, int winc, int rinc) {
-        chain1d_step<R, M, KIND, U>(Rp, Lp, C, wptr, rptr, winc, rinc);
-        if constexpr (U + 1 < M) Chain1dUnroll<R, M, KIND, U + 1>::run(Rp, Lp, C, wptr, rptr, winc, rinc);
+                                               typename Cx<R>::T *&wptr, const typename Cx<R>::T *&rptr, int winc, int rinc,
+                                               Chain1dLinks &lk) {
+        chain1d_step<R, M, KIND, RBL, U>(Rp, Lp, C, wptr, rptr, winc, rinc, lk);
+        if constexpr (U + 1 < M) Chain1dUnroll<R, M, KIND, RBL, U + 1>::run(Rp, Lp, C, wptr, rptr, winc, rinc, lk);
     }
 };
 
@@ -177,7 +223,7 @@ template <typename R, int M> struct Chain1dShape {
         (Chain1dExchange<R>::SMEM ? 2 * Chain1dExchange<R>::AREA : 4 * Chain1dExchange<R>::KMAX);
 };
 
-template <typename R, int M, int KIND>
+template <typename R, int M, int KIND, bool RBL>
 __global__ void __launch_bounds__(Chain1dShape<R, M>::WARPS * 32, Chain1dShape<R, M>::MINB)
 step_chain1d_kernel(const Chain1dArgs<R> a) {
     typedef typename Cx<R>::T V;
@@ -269,17 +315,24 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
             }
             // ---- k steps in registers; the outflow of this tile is recorded for the next one (its left neighbour).
             // The starter (j = 0) reads a record nobody wrote: its inflow is garbage by construction.
+            Chain1dLinks lk;
+            if constexpr (RBL) {
+                long long x0 = X + (long long)lane * M;            // X in (-W, N]: wrap once
+                if (x0 < 0) x0 += N; else if (x0 >= N) x0 -= N;
+                lk.x0 = x0; lk.n_sites = N; lk.t = a.t0; lk.walk = (unsigned)w;
+                lk.key0 = a.rbl_key0; lk.key1 = a.rbl_key1; lk.thr = a.rbl_thr;
+            }
             if constexpr (EX::SMEM) {
                 V *wptr = area + (lane == 0 ? 32 + (j & 1) * (EX::KMAX / 2) : lane);
                 const V *rptr = area + (lane == 31 ? 32 + ((j & 1) ^ 1) * (EX::KMAX / 2) : lane + 1);
                 for (int s = 0; s < a.k; s += M)
-                    Chain1dUnroll<R, M, KIND, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc);
+                    Chain1dUnroll<R, M, KIND, RBL, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc, lk);
             } else {
                 V *wptr = area + (j & 1) * 2 * a.k;
                 const V *rptr = area + ((j & 1) ^ 1) * 2 * a.k;
                 const int rinc2 = (((lane + 1) & 31) << 8) | ((j > 0 && lane == 0) ? 1 : 0);
                 for (int s = 0; s < a.k; s += M) {
-                    Chain1dUnroll<R, M, KIND, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc2);
+                    Chain1dUnroll<R, M, KIND, RBL, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc2, lk);
                     wptr += 2 * M; rptr += 2 * M;
                 }
                 __syncwarp();                              // outflow record complete before the next tile reads it
@@ -338,12 +391,12 @@ int chain1d_max_k(const qw_sim *s) {
 
 // Resident warps of the grid and the dynamic shared memory of one CTA at depth k.  The kernel attribute and the
 // occupancy are taken once per device for the deepest launch, so every depth runs with the same persistent grid.
-template <typename R, int M, int KIND>
+template <typename R, int M, int KIND, bool RBL>
 static int chain1d_grid(const qw_sim *s, int k, int *warps_out, size_t *smem_out) {
     typedef typename Cx<R>::T V;
     constexpr int WARPS = Chain1dShape<R, M>::WARPS;
     const size_t smem_max = (size_t)WARPS * Chain1dShape<R, M>::SMEM_ELEMS * sizeof(V);
-    auto kern = step_chain1d_kernel<R, M, KIND>;
+    auto kern = step_chain1d_kernel<R, M, KIND, RBL>;
     static int ctas_per_sm[64];                                            // per device (cudaFuncSetAttribute is per device)
     const int dev = s->device & 63;
     if (ctas_per_sm[dev] == 0) {
@@ -360,14 +413,14 @@ static int chain1d_grid(const qw_sim *s, int k, int *warps_out, size_t *smem_out
     return ctas_per_sm[dev];
 }
 
-template <typename R, int M, int KIND>
+template <typename R, int M, int KIND, bool RBL>
 static int launch_chain1d_t(qw_sim *s, const void *in, void *out, int k, bool dry, double *cost) {
     typedef typename Cx<R>::T V;
     constexpr int WARPS = Chain1dShape<R, M>::WARPS;
     constexpr int W = 32 * M;
     const Geom &g = s->g;
     int grid_warps = 0; size_t smem = 0;
-    if (chain1d_grid<R, M, KIND>(s, k, &grid_warps, &smem) < 1)
+    if (chain1d_grid<R, M, KIND, RBL>(s, k, &grid_warps, &smem) < 1)
         return fail(QW_ECUDA, "step_chain1d_kernel does not fit on an SM at depth %d", k);
     if (s->max_ctas > 0 && grid_warps > s->max_ctas * WARPS) grid_warps = s->max_ctas * WARPS;
     // chains: as many as the grid has warps (a multiple of them for a batch), each a multiple of 32 sites
@@ -391,15 +444,22 @@ static int launch_chain1d_t(qw_sim *s, const void *in, void *out, int k, bool dr
     a.scale_m = sm;
     long long blocks = (a.total_chains + WARPS - 1) / WARPS;
     if (blocks > grid_warps / WARPS) blocks = grid_warps / WARPS;
-    step_chain1d_kernel<R, M, KIND><<<(unsigned)blocks, WARPS * 32, smem, s->stream>>>(a);
+    a.rbl_key0 = (unsigned)(s->rbl_seed & 0xffffffffu); a.rbl_key1 = (unsigned)(s->rbl_seed >> 32);
+    a.rbl_thr = s->rbl_thr;
+    a.t0 = (unsigned)((unsigned long long)s->t & 0xffffffffu);
+    step_chain1d_kernel<R, M, KIND, RBL><<<(unsigned)blocks, WARPS * 32, smem, s->stream>>>(a);
     QW_LAUNCH_CHECK(s, "step_chain1d_kernel");
     return QW_OK;
 }
 
 template <typename R>
 static int launch_chain1d_r(qw_sim *s, const void *in, void *out, int k, bool dry, double *cost) {
-    if (s->coin_kind == COIN_HADAMARD) return launch_chain1d_t<R, 16, COIN_HADAMARD>(s, in, out, k, dry, cost);
-    return launch_chain1d_t<R, 8, COIN_GENERAL>(s, in, out, k, dry, cost);
+    if (s->rbl) {
+        if (s->coin_kind == COIN_HADAMARD) return launch_chain1d_t<R, 16, COIN_HADAMARD, true>(s, in, out, k, dry, cost);
+        return launch_chain1d_t<R, 8, COIN_GENERAL, true>(s, in, out, k, dry, cost);
+    }
+    if (s->coin_kind == COIN_HADAMARD) return launch_chain1d_t<R, 16, COIN_HADAMARD, false>(s, in, out, k, dry, cost);
+    return launch_chain1d_t<R, 8, COIN_GENERAL, false>(s, in, out, k, dry, cost);
 }
 
 // A ring with a uniform coin, at least two tiles long; k a multiple of the tile granule M, at most chain1d_max_k.
@@ -407,7 +467,7 @@ bool chain1d_eligible(const qw_sim *s, int k) {
     const Geom &g = s->g;
     const int M = chain1d_granule(s);
     return g.dim == 1 && g.boundary == QW_PERIODIC && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
-           !s->rbl && g.en >= 64LL * M && k >= M && k % M == 0 && k <= chain1d_max_k(s);
+           g.en >= 64LL * M && k >= M && k % M == 0 && k <= chain1d_max_k(s);
 }
 
 // Tile computations per warp of one launch (the launch's cost in units of one tile advanced k steps).

@@ -15,12 +15,14 @@ pytestmark = pytest.mark.gpu
 SEED = qi.SEED_RBL
 
 
-def gpu_rbl(qw, w, p, seed, steps, schedule=None, inverse=0, window=True, split=None):
+def gpu_rbl(qw, w, p, seed, steps, schedule=None, inverse=0, window=True, split=None, k=0, options=None):
     h = qw.create_for(w)
     try:
         qw.qw_set_random_broken_links(h, 1, p, seed)
+        for key, value in (options or {}).items():
+            qw.qw_set_option(h, key, value)
         if schedule is not None:
-            qw.qw_set_schedule(h, schedule, 0)
+            qw.qw_set_schedule(h, schedule, k)
         qw.qw_set_window(h, window)
         qw.load_state(h, w)
         if split:
@@ -138,3 +140,34 @@ def test_rbl_multi_tile_lattices(qw, oracle, dev, dtype):
         if w.state is None:                                       # delta start: the window must not change anything
             b = gpu_rbl(qw, w, p, SEED, w.steps, window=False)[0]
             assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("coin", ["hadamard", "su2"])
+def test_rbl_inside_the_temporally_blocked_ring_kernel(qw, oracle, dev, dtype, coin):
+    """Random broken links inside the chained blocked 1D kernel (qw_step_chain1d.cu): one Philox call per (site, step)
+    in registers, a broken link = a predicated swap of two registers of the lane.  Rings of several chains / tiles with
+    ragged ends and a batch, every depth, split stepping (the step index carries over), p = 0.1 and 0.5: the same links as
+    the oracle, and the same state as the fused-RBL kernel (bit for bit for a general coin; <= 4 ulp per step for the
+    Hadamard coin, whose scale the blocked kernel applies once per 16 steps)."""
+    rng = np.random.default_rng(45)
+    for sites, steps, k, batch, max_ctas, p in ((20000, 112, 48, 1, 1, 0.1), (3001, 64, 16, 3, 2, 0.5), (70001, 80, 0, 1, 0, 0.1)):
+        c = qi.hadamard(dtype) if coin == "hadamard" else qi.su2(*rng.uniform(0, 2 * np.pi, 3)).astype(dtype)
+        w = qi.Workload("rblchain", 1, (sites,), batch, qi.PERIODIC, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
+                        state=qi.random_state(12, batch, sites, 2, dtype, normalise_per_walk=True))
+        opt = {qw.QW_OPT_MAX_CTAS: max_ctas, qw.QW_OPT_BLOCKED1D_KERNEL: 2}
+        b, mom, sched, t = gpu_rbl(qw, w, p, SEED, steps, schedule=qw.QW_SCHED_BLOCKED, k=k, options=opt)
+        assert sched == qw.QW_SCHED_BLOCKED and t == steps
+        f = gpu_rbl(qw, w, p, SEED, steps, schedule=qw.QW_SCHED_FUSED)[0]
+        if coin == "su2":
+            assert np.array_equal(b, f), (sites, steps, k)
+        else:
+            eps = np.finfo(np.float64 if dtype == np.complex128 else np.float32).eps
+            assert np.max(np.abs(b.astype(np.complex128) - f.astype(np.complex128))) <= 4 * eps * steps * float(np.max(np.abs(f)))
+        close(w, b, oracle_rbl(oracle, w, p, SEED, steps))
+        s2 = gpu_rbl(qw, w, p, SEED, steps, schedule=qw.QW_SCHED_BLOCKED, k=k, options=opt, split=steps // 2 // 16 * 16)[0]
+        assert np.array_equal(b, s2)
+        if dtype == np.complex128:
+            assert np.max(np.abs(mom[:, 0] - 1)) < 1e-12
+    auto = gpu_rbl(qw, w, p, SEED, steps)                             # AUTO takes the blocked kernel on a long ring
+    assert auto[2] == qw.QW_SCHED_BLOCKED and np.array_equal(auto[0], b)
