@@ -36,8 +36,10 @@
 //              link    = (owner site, axis): the owner is the end from which the link points in the
 //                        positive direction (dm > 0, or dm = 0 and dn > 0); axis = 0 for links along n
 //                        (natural / 1D) or along (+1,+1) (diagonal), 1 for links along m or (+1,-1)
-//              counter = (owner index low 32 bits, owner index high bits, step t, walk w), key = seed
-//              broken  iff output word [axis] < floor(p * 2^32)
+//              number  = owner index * dim + axis   (dim = links owned per site: 1 in 1D, 2 in 2D)
+//              counter = (number / 4 low 32 bits, number / 4 high bits, step t, walk w), key = seed
+//              broken  iff output word [number mod 4] < floor(p * 2^32)
+//            (one generator call yields four independent words: it serves four consecutive links)
 //            Links that leave an open lattice stay broken regardless.  Both ends of a link evaluate the
 //            same function, so U(t) is unitary (pinned by the dense form).
 //
@@ -131,12 +133,16 @@ inline bool rbl_broken(const Lattice& L, int64_t w, int64_t m, int64_t n, int a,
     int axis;
     if (dm != 0 && dn != 0) axis = (dm * dn > 0) ? 0 : 1;      // diagonal lattice
     else axis = (dm != 0) ? 1 : 0;                             // natural lattice / 1D
-    const uint32_t ctr[4] = { (uint32_t)((uint64_t)owner & 0xffffffffu), (uint32_t)((uint64_t)owner >> 32),
+    // link number: the links of a walk are numbered owner * (links owned per site) + axis; one generator call serves
+    // the four links 4g .. 4g+3 with its four output words (reading R27)
+    const uint64_t link = (uint64_t)owner * (uint64_t)L.dim + (uint64_t)axis;
+    const uint64_t group = link >> 2;
+    const uint32_t ctr[4] = { (uint32_t)(group & 0xffffffffu), (uint32_t)(group >> 32),
                               (uint32_t)((uint64_t)t & 0xffffffffu), (uint32_t)((uint64_t)w & 0xffffffffu) };
     const uint32_t key[2] = { (uint32_t)(seed & 0xffffffffu), (uint32_t)(seed >> 32) };
     uint32_t out[4];
     philox4x32_10(ctr, key, out);
-    return (uint64_t)out[axis] < thr;
+    return (uint64_t)out[link & 3u] < thr;
 }
 
 inline uint64_t rbl_threshold(double p) {       // floor(p * 2^32), p in [0, 1]

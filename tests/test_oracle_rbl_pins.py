@@ -139,6 +139,36 @@ def test_p0_is_the_plain_walk_and_p1_freezes_the_walker(oracle, dim):
     assert np.allclose(np.sum(np.abs(c) ** 2, axis=2), np.sum(np.abs(psi0) ** 2, axis=2), rtol=0, atol=1e-15)
 
 
+@pytest.mark.parametrize("dim,lattice", [(1, 0), (2, 0), (2, 1)])
+def test_link_states_are_the_documented_function_of_the_generator(oracle, dim, lattice):
+    """Reading R27, written out: link number = owner * dim + axis, counter = (number // 4, 0, t, walk), key = seed,
+    broken iff word[number % 4] < floor(p 2^32).  The mask the oracle's stepper uses must be exactly that function of
+    the generator (which the known-answer vectors pin): a wrong word index, owner or axis fails here."""
+    ext = (23,) if dim == 1 else (5, 7)
+    em, en = (1, ext[0]) if dim == 1 else ext
+    p, seed, t, batch = 0.37, 0x0123456789ABCDEF, 5, 2
+    thr = int(p * 2 ** 32)
+    key = [seed & 0xffffffff, seed >> 32]
+    mask = oracle.rbl_mask(ext, p, seed, t, boundary=0, batch=batch, lattice=lattice).reshape(batch, em, en, 2 * dim)
+    if dim == 1:
+        dirs = [(0, 1), (0, -1)]
+    elif lattice == 0:
+        dirs = [(0, 1), (1, 0), (-1, 0), (0, -1)]            # PAPER.md:88 eq. 8, c = 2j + k
+    else:
+        dirs = [(1, 1), (1, -1), (-1, 1), (-1, -1)]          # PAPER.md:106 Fig. 1c
+    for w in range(batch):
+        for m in range(em):
+            for n in range(en):
+                for a, (dm, dn) in enumerate(dirs):
+                    tm, tn = (m + dm) % em, (n + dn) % en
+                    positive = dm > 0 or (dm == 0 and dn > 0)
+                    owner = (m * en + n) if positive else (tm * en + tn)
+                    axis = (0 if dm * dn > 0 else 1) if (dm != 0 and dn != 0) else (1 if dm != 0 else 0)
+                    number = owner * dim + axis
+                    word = oracle.philox4x32_10([number // 4, 0, t, w], key)[number % 4]
+                    assert mask[w, m, n, a] == (1 if int(word) < thr else 0), (w, m, n, a)
+
+
 def test_batch_members_and_start_times_are_addressed_by_the_counter(oracle):
     """Walk w of a batch sees the links of counter word 3 = w; starting at t0 sees those of steps t0, t0+1, ..."""
     rng = np.random.default_rng(6)
