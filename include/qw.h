@@ -140,8 +140,10 @@ int qw_set_broken_links(qw_sim *s, const uint8_t *mask);
  * applies U(t) in which every link of the lattice is broken independently with probability p in [0, 1];
  * a broken link acts as in qw_set_broken_links.  The paper names no generator; the state of a link is
  * the pure function (reading R27)
- *     broken  <=>  Philox4x32-10(counter = (owner lo32, owner hi32, t lo32, walk lo32), key = seed)[axis]
+ *     number  =  owner * dim + axis                      (dim = links a site owns: 1 in 1D, 2 in 2D)
+ *     broken  <=>  Philox4x32-10(counter = (number/4 lo32, number/4 hi32, t lo32, walk lo32), key = seed)[number mod 4]
  *                  < floor(p * 2^32)
+ * (one generator call serves four consecutive links with its four output words).
  * owner = site index of the end from which the link points in the positive direction (dm > 0, or
  * dm = 0 and dn > 0); axis = 0 for links along n (1D, natural) or along (+1,+1) (diagonal), 1 for links
  * along m or along (+1,-1).  Both ends of a link see the same value, so every U(t) is unitary, and

@@ -50,14 +50,13 @@ template <typename R, int DIM> struct FusedShape {
 // at step a.t?  The link is named by its OWNER (the end from which it points in the positive direction: dm > 0, or
 // dm = 0 and dn > 0) and its axis (0: along n / along (+1,+1); 1: along m / along (+1,-1)), so that both ends of a
 // link evaluate the same function and U(t) stays unitary (eq. 9: RBL is a property of the link).
-template <typename A>
+template <int DIM_LINKS, typename A>
 __device__ __forceinline__ bool rbl_link_broken(const A &a, long long w, long long m, long long n, long long tm,
                                                 long long tn, int dm, int dn) {
     const bool positive = dm > 0 || (dm == 0 && dn > 0);
     const unsigned long long owner = (unsigned long long)(positive ? (m * a.en + n) : (tm * a.en + tn));
     const int axis = (dm != 0 && dn != 0) ? ((dm * dn > 0) ? 0 : 1) : (dm != 0 ? 1 : 0);
-    const unsigned word = philox4x32_10_word((unsigned)owner, (unsigned)(owner >> 32), a.t, (unsigned)w,
-                                             a.rbl_key0, a.rbl_key1, axis);
+    const unsigned word = rbl_link_word(owner * (DIM_LINKS) + (unsigned)axis, a.t, (unsigned)w, a.rbl_key0, a.rbl_key1);
     return (unsigned long long)word < a.rbl_thr;
 }
 
@@ -99,9 +98,21 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
         for (int u = 0; u < U; ++u) {
             own[u] = 0;
             if (live[u]) {
+                // the links this site owns: numbers owner * DIM + axis (1D: word owner & 3 of call owner / 4; 2D: words
+                // 2 (owner & 1) + axis of call owner / 2)
                 const unsigned long long owner = (unsigned long long)(m * a.en + a.n_lo + n_base + (long long)u * BS);
+                unsigned wd[4];
+                rbl_group_words((owner * DIM) >> 2, a.t, (unsigned)w, a.rbl_key0, a.rbl_key1, wd);
                 unsigned w0, w1;
-                philox4x32_10_words01((unsigned)owner, (unsigned)(owner >> 32), a.t, (unsigned)w, a.rbl_key0, a.rbl_key1, w0, w1);
+                if constexpr (DIM == 1) {
+                    const unsigned sel = (unsigned)owner & 3u;
+                    w0 = sel == 0 ? wd[0] : (sel == 1 ? wd[1] : (sel == 2 ? wd[2] : wd[3]));
+                    w1 = 0xffffffffu;                        // no second axis in 1D
+                } else {
+                    const bool odd = ((unsigned)owner & 1u) != 0;
+                    w0 = odd ? wd[2] : wd[0];
+                    w1 = odd ? wd[3] : wd[1];
+                }
                 own[u] = ((unsigned long long)w0 < a.rbl_thr ? 1u : 0u) | ((unsigned long long)w1 < a.rbl_thr ? 2u : 0u);
             }
             link_n[u][threadIdx.x] = (unsigned char)(own[u] & 1u);
@@ -147,7 +158,7 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
             }
             if constexpr (!FAST) {
                 if (a.broken && a.broken[(w * a.sites + x) * CD + c]) stay = true;
-                if (a.rbl && !stay && rbl_link_broken(a, w, m, n, tm, tn, dm, dn)) stay = true;
+                if (a.rbl && !stay && rbl_link_broken<DIM>(a, w, m, n, tm, tn, dm, dn)) stay = true;
             } else if constexpr (SHARE) {
                 if (!stay) {
                     bool broken;
@@ -156,12 +167,12 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
                     else if (dm == 0) {                                                    // the left neighbour's link
                         if (threadIdx.x > 0) broken = link_n[u][threadIdx.x - 1] != 0;
                         else if (u > 0) broken = link_n[u > 0 ? u - 1 : 0][BS - 1] != 0;
-                        else broken = rbl_link_broken(a, w, m, n, tm, tn, dm, dn);         // first site of the block
-                    } else broken = rbl_link_broken(a, w, m, n, tm, tn, dm, dn);           // the upper row's link
+                        else broken = rbl_link_broken<DIM>(a, w, m, n, tm, tn, dm, dn);         // first site of the block
+                    } else broken = rbl_link_broken<DIM>(a, w, m, n, tm, tn, dm, dn);           // the upper row's link
                     if (broken) stay = true;
                 }
             } else if constexpr (RBL) {
-                if (!stay && rbl_link_broken(a, w, m, n, tm, tn, dm, dn)) stay = true;
+                if (!stay && rbl_link_broken<DIM>(a, w, m, n, tm, tn, dm, dn)) stay = true;
             }
             const long long dst = stay ? ((CD - 1 - c) * a.plane_stride + row_off + n)
                                        : (c * a.plane_stride + w * a.walk_stride + tm * a.pitch + tn);
@@ -200,7 +211,7 @@ step_inverse_kernel(const StepArgs<R, 2 * DIM> a) {
             if (DIM == 2) stay |= (tm < 0) | (tm >= a.em);
         }
         if (a.broken && a.broken[(w * a.sites + x) * CD + c]) stay = true;
-        if (a.rbl && !stay && rbl_link_broken(a, w, m, n, tm, tn, dm, dn)) stay = true;
+        if (a.rbl && !stay && rbl_link_broken<DIM>(a, w, m, n, tm, tn, dm, dn)) stay = true;
         const long long src = stay ? ((CD - 1 - c) * a.plane_stride + row_off + n)
                                    : (c * a.plane_stride + w * a.walk_stride + tm * a.pitch + tn);
         v[c] = cx_load<R>(a.in + src);

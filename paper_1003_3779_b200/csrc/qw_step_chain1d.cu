@@ -128,13 +128,33 @@ __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M],
         Lp[p] = v[1];
     }
     constexpr int P0 = (2 * U) % M, P1 = (2 * U + 1) % M;
-    [[maybe_unused]] auto link_broken = [&](int q) -> bool {      // link owned by the site at logical position q
-        long long x = lk.x0 + q;
-        if (x >= lk.n_sites) x -= lk.n_sites;
-        const unsigned word = philox4x32_10_word((unsigned)x, (unsigned)((unsigned long long)x >> 32), lk.t, lk.walk,
-                                                 lk.key0, lk.key1, 0);
-        return (unsigned long long)word < lk.thr;
-    };
+    // bit q of `bits`: the link owned by the site at logical position q (site x0 + q; in 1D link number = site index) is
+    // broken at this step.  One generator call serves the four links 4g .. 4g+3 (reading R27), so a lane's M
+    // consecutive sites need M/4 + 1 calls; a lane that straddles the seam of the ring takes one call per site.
+    unsigned bits = 0;
+    if constexpr (RBL) {
+        if (lk.x0 + M <= lk.n_sites) {
+            const unsigned long long g0 = (unsigned long long)lk.x0 >> 2;
+            unsigned long long wide = 0;                           // bit 4 gi + wd: word wd of group g0 + gi
+#pragma unroll
+            for (int gi = 0; gi < M / 4 + 1; ++gi) {
+                unsigned wd[4];
+                rbl_group_words(g0 + gi, lk.t, lk.walk, lk.key0, lk.key1, wd);
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    wide |= (unsigned long long)((unsigned long long)wd[i] < lk.thr ? 1u : 0u) << (4 * gi + i);
+            }
+            bits = (unsigned)(wide >> ((unsigned)lk.x0 & 3u));
+        } else {
+#pragma unroll 1
+            for (int q = 0; q < M; ++q) {
+                long long x = lk.x0 + q;
+                if (x >= lk.n_sites) x -= lk.n_sites;
+                bits |= ((unsigned long long)rbl_link_word((unsigned long long)x, lk.t, lk.walk, lk.key0, lk.key1) < lk.thr ? 1u : 0u) << q;
+            }
+        }
+    }
+    [[maybe_unused]] auto link_broken = [&](int q) -> bool { return (bits >> q) & 1u; };
     if constexpr (RBL) {
 #pragma unroll
         for (int q = 0; q + 1 < M; ++q) {
