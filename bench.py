@@ -54,6 +54,17 @@ def make_workload(name: str, walk_steps=None):
         return qi.k4(steps=walk_steps)
     if name == "k0":
         return qi.k0(steps=walk_steps or 100)
+    if name == "dis":
+        # coin families on a long lattice (SURVEY.md 8(a) A8 beyond the resident kernel; eq. 1): 4 rings of
+        # 2^24 sites, each with its own SU(2) coin and per-site phase disorder (BASELINE.json:configs[4]'s family)
+        n, batch = 1 << 24, 4
+        rng = np.random.default_rng(qi.SEED_K4)
+        ang = rng.uniform(0.0, 2 * np.pi, (batch, 3))
+        phi = rng.uniform(0.0, 2 * np.pi, (batch, n))
+        return qi.Workload("DIS", 1, (n,), batch, qi.PERIODIC, np.dtype(np.complex128), walk_steps or 192, qi.COIN_PER_WALK,
+                           qi.su2(ang[:, 0], ang[:, 1], ang[:, 2]), phases=np.exp(1j * phi),
+                           state=qi.random_state(qi.SEED_K4 + 1, batch, n, 2, np.complex128, normalise_per_walk=True),
+                           outputs=("moments",))
     if name == "seg":
         # NEXT-3: the paper's Fig. 3-left "segment": an open 1D Hadamard segment with
         # the delta start of K0, run for five times its length so that the front reflects off the walls (A3, PAPER.md:94-101
@@ -256,6 +267,13 @@ def aggregate_rate(units_per_rank: float, ms_per_rank: float, world: int, device
 
 
 # ----------------------------------------------------------------------------------------------
+def dataclasses_replace_ring(w, n):
+    """The first walk of a ring workload, cut to its first n sites (inputs for the oracle's bounded sample)."""
+    import dataclasses
+    return dataclasses.replace(w, extents=(n,), batch=1, coin=np.ascontiguousarray(w.coin[:1]),
+                               phases=np.ascontiguousarray(w.phases[:1, :n]), state=np.ascontiguousarray(w.state[:1, :n]))
+
+
 def cpu_model():
     try:
         with open("/proc/cpuinfo") as f:
@@ -296,6 +314,9 @@ def oracle_sample(name: str, w, seconds_target: float = 15.0):
     if name == "k4":
         sw = qi.k4(batch=256, half=1024, steps=1)        # the per-site matrices of all 4096 walks would be 537 MB x 2
         desc = "256 of the 4096 walks, full length of each, %d walk steps"
+    elif name == "dis":
+        sw = dataclasses_replace_ring(w, 1 << 22)             # per-site matrices of the full workload would be 4 GiB
+        desc = "one of the 4 rings cut to 2^22 sites, %d walk steps"
     elif name in ("k0", "seg", "t1"):
         desc = "the whole lattice, %d walk steps"
     else:
@@ -337,7 +358,7 @@ def run_reference(args):
     else:
         sw = {"k2": lambda: qi.k2(half=512, steps=2), "k3hxh": lambda: qi.k3(extent=1024, steps=2, coin="hxh"),
               "k3dft": lambda: qi.k3(extent=1024, steps=2, coin="dft"), "k4": lambda: qi.k4(batch=64, steps=16),
-              "k0": lambda: qi.k0(), "seg": lambda: make_workload("seg", 1000),
+              "k0": lambda: qi.k0(), "seg": lambda: make_workload("seg", 1000), "dis": lambda: qi.k4(batch=64, steps=16),
               "t1": lambda: make_workload("t1", 8), "t2": lambda: make_workload("t2", 8)}[args.workload]()
         sample = "%s cut to %d sites x batch %d, %d walk steps per bench step" % (sw.name, sw.sites, sw.batch, sw.steps)
         full_sites, full_batch, full_steps = sw.sites, sw.batch, sw.steps
@@ -400,7 +421,8 @@ def run_gpu(args):
     real = np.float64 if w.dtype == np.complex128 else np.float32
     ebytes = np.dtype(w.dtype).itemsize
     site_updates_per_step = float(w.sites) * w.batch * w.steps
-    alg_bytes_per_site = 2 * w.coin_dim * ebytes          # read + write every amplitude once
+    # read + write every amplitude once (+ the site's phase where the coin family has one)
+    alg_bytes_per_site = 2 * w.coin_dim * ebytes + (ebytes if w.phases is not None else 0)
 
     h = qw.create_for(w)
     if args.schedule is not None:
@@ -640,7 +662,7 @@ def main():
                     help="timed bench steps (default: as many as make the timed region last about 2 s, at least 3)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="k1", choices=["k0", "k1", "k1c64", "k2", "k3hxh", "k3dft", "k4", "seg", "t1", "t2"])
+    ap.add_argument("--workload", default="k1", choices=["k0", "k1", "k1c64", "k2", "k3hxh", "k3dft", "k4", "seg", "dis", "t1", "t2"])
     ap.add_argument("--walk-steps", type=int, default=None, help="walk steps per bench step (default: the config's)")
     ap.add_argument("--schedule", default=None, choices=["auto", "generic", "fused", "blocked", "resident", "tiled"])
     ap.add_argument("--k", type=int, default=0)

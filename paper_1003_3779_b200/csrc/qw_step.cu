@@ -60,7 +60,9 @@ __device__ __forceinline__ bool rbl_link_broken(const A &a, long long w, long lo
     return (unsigned long long)word < a.rbl_thr;
 }
 
-template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK, bool DIAG = false>
+// FAM (with FAST): the coin FAMILY of PAPER.md:35-38 eq. 1 on the vectorised path — a per-walk matrix (read once per
+// thread: all sites of a block belong to one walk) and / or the per-site phase table as a third, coalesced read stream.
+template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK, bool DIAG = false, bool FAM = false>
 __global__ void __launch_bounds__(BS)
 step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
     constexpr int CD = 2 * DIM;
@@ -124,7 +126,22 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
         if (!live[u]) continue;
         const long long n = a.n_lo + n_base + (long long)u * BS;
         const long long x = m * a.en + n;
-        if constexpr (FAST) {
+        if constexpr (FAST && FAM) {
+            if (a.coin_mode == QW_COIN_PER_WALK) {
+                const R *Cg = reinterpret_cast<const R *>(a.coins + w * (CD * CD));
+                R C[2 * CD * CD];
+#pragma unroll
+                for (int i = 0; i < 2 * CD * CD; ++i) C[i] = Cg[i];
+                apply_coin<R, CD, COIN_GENERAL>(C, v[u]);
+            } else {
+                apply_coin<R, CD, KIND>(a.coin, v[u]);
+            }
+            if (a.phases) {
+                const cplx<R> ph = cx_load<R>(a.phases + w * a.sites + x);
+#pragma unroll
+                for (int c = 0; c < CD; ++c) v[u][c] = cx_mul(ph.re, ph.im, v[u][c]);
+            }
+        } else if constexpr (FAST) {
             apply_coin<R, CD, KIND>(a.coin, v[u]);
         } else {
             if (a.coin_mode == QW_COIN_UNIFORM) {
@@ -257,14 +274,14 @@ static void fill_args(const qw_sim *s, const void *in, void *out, const Box &box
     for (int i = 0; i < 2 * g.cdim * g.cdim; ++i) a.coin[i] = (R)s->h_coin[i];
 }
 
-template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK, bool DIAG = false>
+template <typename R, int DIM, int KIND, bool FAST, int U, bool RBL = false, int BS = STEP_BLOCK, bool DIAG = false, bool FAM = false>
 static int launch_scatter(qw_sim *s, StepArgs<R, 2 * DIM> &a) {
     const long long per_block = (long long)BS * U;
     a.chunks_per_row = (int)((a.box_n + per_block - 1) / per_block);
     const long long blocks = s->g.batch * a.box_m * a.chunks_per_row;
     if (blocks <= 0) return QW_OK;
     if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
-    step_scatter_kernel<R, DIM, KIND, FAST, U, RBL, BS, DIAG><<<(unsigned)blocks, BS, 0, s->stream>>>(a);
+    step_scatter_kernel<R, DIM, KIND, FAST, U, RBL, BS, DIAG, FAM><<<(unsigned)blocks, BS, 0, s->stream>>>(a);
     QW_LAUNCH_CHECK(s, "step_scatter_kernel");
     return QW_OK;
 }
@@ -287,6 +304,22 @@ static int launch_step_t(qw_sim *s, const void *in, void *out, const Box &box, b
     StepArgs<R, 2 * DIM> a;
     fill_args<R, DIM>(s, in, out, box, a);
     const bool fast = allow_fast && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken;
+    // coin families on the vectorised path: per-walk matrices and / or site phases (natural lattice, no links)
+    const bool fam = allow_fast && !fast && s->coin_mode != QW_COIN_PER_SITE && !s->d_broken && !s->rbl &&
+                     s->g.lattice == QW_NATURAL;
+    if (fam) {
+        constexpr int UF = FusedShape<R, DIM>::U, BS = FusedShape<R, DIM>::BS;
+        if (s->coin_mode == QW_COIN_UNIFORM) {         // uniform matrix + phases: keep the named coin's evaluation
+            switch (s->coin_kind) {
+                case COIN_HADAMARD: if (DIM == 1) return launch_scatter<R, DIM, COIN_HADAMARD, true, UF, false, BS, false, true>(s, a); break;
+                case COIN_GROVER4:  if (DIM == 2) return launch_scatter<R, DIM, COIN_GROVER4, true, UF, false, BS, false, true>(s, a); break;
+                case COIN_HXH4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_HXH4, true, UF, false, BS, false, true>(s, a); break;
+                case COIN_DFT4:     if (DIM == 2) return launch_scatter<R, DIM, COIN_DFT4, true, UF, false, BS, false, true>(s, a); break;
+                default: break;
+            }
+        }
+        return launch_scatter<R, DIM, COIN_GENERAL, true, UF, false, BS, false, true>(s, a);
+    }
     if (fast) {
         if constexpr (DIM == 2) {
             if (s->g.lattice == QW_DIAGONAL)

@@ -44,6 +44,17 @@ struct Chain1dArgs {
     unsigned rbl_key0, rbl_key1;
     unsigned long long rbl_thr;     // floor(p * 2^32)
     unsigned t0;                    // step index of the first step of this launch (low 32 bits)
+    // coin family (FAM template instances only; eq. 1): per-walk matrices and / or per-site phases
+    const typename Cx<R>::T *coins;     // [walk][2][2], or nullptr (uniform coin)
+    const typename Cx<R>::T *phases;    // [walk][site], or nullptr
+};
+
+// What the FAM instances carry through the steps: the phases of the lane's M sites (renamed like the L plane, one site
+// per step: logical q of step t lives in ph[(q + t) mod M]) and where the next one comes from.
+template <typename R, int M> struct Chain1dPhases {
+    cplx<R> ph[M];
+    const typename Cx<R>::T *row;   // phases of this walk
+    long long next, n_sites;        // site whose phase enters the lane at the end of the current step
 };
 
 // What the RBL instances carry through the steps: the lattice coordinate of the lane's logical site 0 and the counter words.
@@ -102,12 +113,20 @@ template <typename R> struct Chain1dExchange {
 // i.e. the pair (R'[Q], L'[Q - 1]) = (phi_R[Q], phi_L[Q + 1]) is SWAPPED.  In this frame both members of the pair sit in
 // the same lane — Rp[q] and the register that holds phi_L[q + 1] (for q = M - 1: the one just received from the lane
 // above) — so a broken link is a predicated swap of two registers; its state is one Philox call per (site, step).
-template <typename R, int M, int KIND, bool RBL, int U>
+//
+// FAM (coin family): phi = ph_x * (C_w psi) with the phase of the site (BASELINE.json:configs[4]).  The frame moves one
+// site per step, so the lane's phases are renamed like a plane that moves one site per step, and the phase of the one site
+// that enters the lane is read from global memory a step ahead (each phase is read once per tile: lane-strided, L2).
+template <typename R, int M, int KIND, bool RBL, bool FAM, int U>
 __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
                                              typename Cx<R>::T *&wptr, const typename Cx<R>::T *&rptr, int winc, int rinc,
-                                             Chain1dLinks &lk) {
+                                             Chain1dLinks &lk, Chain1dPhases<R, FAM ? M : 1> &ps) {
     typedef typename Cx<R>::T V;
     typedef Chain1dExchange<R> EX;
+    [[maybe_unused]] V ph_next;
+    if constexpr (FAM) {
+        if (ps.row) ph_next = ps.row[ps.next];
+    }
 #pragma unroll
     for (int q = 0; q < M; ++q) {
         const int p = (q + 2 * U) % M;
@@ -124,8 +143,21 @@ __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M],
         } else {
             apply_coin<R, 2, KIND>(C, v);
         }
+        if constexpr (FAM) {
+            if (ps.row) {
+                const cplx<R> ph = ps.ph[(q + U) % (FAM ? M : 1)];
+                v[0] = cx_mul(ph.re, ph.im, v[0]);
+                v[1] = cx_mul(ph.re, ph.im, v[1]);
+            }
+        }
         Rp[q] = v[0];
         Lp[p] = v[1];
+    }
+    if constexpr (FAM) {
+        if (ps.row) {                                             // logical site 0 leaves the lane, a new logical M-1 enters
+            ps.ph[U % (FAM ? M : 1)] = cplx<R>{ph_next.x, ph_next.y};
+            ps.next = ps.next + 1 == ps.n_sites ? 0 : ps.next + 1;
+        }
     }
     constexpr int P0 = (2 * U) % M, P1 = (2 * U + 1) % M;
     // bit q of `bits`: the link owned by the site at logical position q (site x0 + q; in 1D link number = site index) is
@@ -197,13 +229,13 @@ __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M],
     }
 }
 
-template <typename R, int M, int KIND, bool RBL, int U>
+template <typename R, int M, int KIND, bool RBL, bool FAM, int U>
 struct Chain1dUnroll {
     static __device__ __forceinline__ void run(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M], const R *C,
                                                typename Cx<R>::T *&wptr, const typename Cx<R>::T *&rptr, int winc, int rinc,
-                                               Chain1dLinks &lk) {
-        chain1d_step<R, M, KIND, RBL, U>(Rp, Lp, C, wptr, rptr, winc, rinc, lk);
-        if constexpr (U + 1 < M) Chain1dUnroll<R, M, KIND, RBL, U + 1>::run(Rp, Lp, C, wptr, rptr, winc, rinc, lk);
+                                               Chain1dLinks &lk, Chain1dPhases<R, FAM ? M : 1> &ps) {
+        chain1d_step<R, M, KIND, RBL, FAM, U>(Rp, Lp, C, wptr, rptr, winc, rinc, lk, ps);
+        if constexpr (U + 1 < M) Chain1dUnroll<R, M, KIND, RBL, FAM, U + 1>::run(Rp, Lp, C, wptr, rptr, winc, rinc, lk, ps);
     }
 };
 
@@ -243,7 +275,7 @@ template <typename R, int M> struct Chain1dShape {
         (Chain1dExchange<R>::SMEM ? 2 * Chain1dExchange<R>::AREA : 4 * Chain1dExchange<R>::KMAX);
 };
 
-template <typename R, int M, int KIND, bool RBL>
+template <typename R, int M, int KIND, bool RBL, bool FAM = false>
 __global__ void __launch_bounds__(Chain1dShape<R, M>::WARPS * 32, Chain1dShape<R, M>::MINB)
 step_chain1d_kernel(const Chain1dArgs<R> a) {
     typedef typename Cx<R>::T V;
@@ -335,6 +367,28 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
             }
             // ---- k steps in registers; the outflow of this tile is recorded for the next one (its left neighbour).
             // The starter (j = 0) reads a record nobody wrote: its inflow is garbage by construction.
+            Chain1dPhases<R, FAM ? M : 1> ps;
+            if constexpr (FAM) {
+                if (a.coins) {                                     // the walk's own matrix (uniform otherwise)
+                    const R *Cg = reinterpret_cast<const R *>(a.coins + w * 4);
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) C[i] = Cg[i];
+                }
+                ps.row = a.phases ? a.phases + w * N : nullptr;
+                ps.n_sites = N;
+                long long x0 = X + (long long)lane * M;
+                if (x0 < 0) x0 += N; else if (x0 >= N) x0 -= N;
+                if (ps.row) {
+#pragma unroll
+                    for (int q = 0; q < M; ++q) {
+                        long long x = x0 + q;
+                        if (x >= N) x -= N;
+                        const V z = ps.row[x];
+                        ps.ph[q % (FAM ? M : 1)] = cplx<R>{z.x, z.y};
+                    }
+                }
+                ps.next = x0 + M >= N ? x0 + M - N : x0 + M;
+            }
             Chain1dLinks lk;
             if constexpr (RBL) {
                 long long x0 = X + (long long)lane * M;            // X in (-W, N]: wrap once
@@ -346,13 +400,13 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
                 V *wptr = area + (lane == 0 ? 32 + (j & 1) * (EX::KMAX / 2) : lane);
                 const V *rptr = area + (lane == 31 ? 32 + ((j & 1) ^ 1) * (EX::KMAX / 2) : lane + 1);
                 for (int s = 0; s < a.k; s += M)
-                    Chain1dUnroll<R, M, KIND, RBL, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc, lk);
+                    Chain1dUnroll<R, M, KIND, RBL, FAM, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc, lk, ps);
             } else {
                 V *wptr = area + (j & 1) * 2 * a.k;
                 const V *rptr = area + ((j & 1) ^ 1) * 2 * a.k;
                 const int rinc2 = (((lane + 1) & 31) << 8) | ((j > 0 && lane == 0) ? 1 : 0);
                 for (int s = 0; s < a.k; s += M) {
-                    Chain1dUnroll<R, M, KIND, RBL, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc2, lk);
+                    Chain1dUnroll<R, M, KIND, RBL, FAM, 0>::run(Rp, Lp, C, wptr, rptr, winc, rinc2, lk, ps);
                     wptr += 2 * M; rptr += 2 * M;
                 }
                 __syncwarp();                              // outflow record complete before the next tile reads it
@@ -401,7 +455,13 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
 
 // ---- host side ---------------------------------------------------------------------------------------------------
 
-int chain1d_granule(const qw_sim *s) { return s->coin_kind == COIN_HADAMARD ? 16 : 8; }
+// a coin family the FAM instance handles: per-walk matrices and / or site phases on a general (not Hadamard-classified)
+// matrix — the general evaluation, so that the result stays bit-identical to the generic kernel
+static bool chain1d_family(const qw_sim *s) {
+    if (s->coin_mode == QW_COIN_PER_WALK) return true;
+    return s->coin_mode == QW_COIN_UNIFORM && s->d_phases != nullptr && s->coin_kind == COIN_GENERAL;
+}
+int chain1d_granule(const qw_sim *s) { return (s->coin_kind == COIN_HADAMARD && s->coin_mode == QW_COIN_UNIFORM) ? 16 : 8; }
 // deepest launch: what the outflow records hold (Chain1dExchange::KMAX), and k <= W/2 = 16*M for the starter tile
 int chain1d_max_k(const qw_sim *s) {
     const int kmax = s->dtype == QW_C128 ? Chain1dExchange<double>::KMAX : Chain1dExchange<float>::KMAX;
@@ -411,12 +471,12 @@ int chain1d_max_k(const qw_sim *s) {
 
 // Resident warps of the grid and the dynamic shared memory of one CTA at depth k.  The kernel attribute and the
 // occupancy are taken once per device for the deepest launch, so every depth runs with the same persistent grid.
-template <typename R, int M, int KIND, bool RBL>
+template <typename R, int M, int KIND, bool RBL, bool FAM>
 static int chain1d_grid(const qw_sim *s, int k, int *warps_out, size_t *smem_out) {
     typedef typename Cx<R>::T V;
     constexpr int WARPS = Chain1dShape<R, M>::WARPS;
     const size_t smem_max = (size_t)WARPS * Chain1dShape<R, M>::SMEM_ELEMS * sizeof(V);
-    auto kern = step_chain1d_kernel<R, M, KIND, RBL>;
+    auto kern = step_chain1d_kernel<R, M, KIND, RBL, FAM>;
     static int ctas_per_sm[64];                                            // per device (cudaFuncSetAttribute is per device)
     const int dev = s->device & 63;
     if (ctas_per_sm[dev] == 0) {
@@ -433,14 +493,14 @@ static int chain1d_grid(const qw_sim *s, int k, int *warps_out, size_t *smem_out
     return ctas_per_sm[dev];
 }
 
-template <typename R, int M, int KIND, bool RBL>
+template <typename R, int M, int KIND, bool RBL, bool FAM = false>
 static int launch_chain1d_t(qw_sim *s, const void *in, void *out, int k, bool dry, double *cost) {
     typedef typename Cx<R>::T V;
     constexpr int WARPS = Chain1dShape<R, M>::WARPS;
     constexpr int W = 32 * M;
     const Geom &g = s->g;
     int grid_warps = 0; size_t smem = 0;
-    if (chain1d_grid<R, M, KIND, RBL>(s, k, &grid_warps, &smem) < 1)
+    if (chain1d_grid<R, M, KIND, RBL, FAM>(s, k, &grid_warps, &smem) < 1)
         return fail(QW_ECUDA, "step_chain1d_kernel does not fit on an SM at depth %d", k);
     if (s->max_ctas > 0 && grid_warps > s->max_ctas * WARPS) grid_warps = s->max_ctas * WARPS;
     // chains: as many as the grid has warps (a multiple of them for a batch), each a multiple of 32 sites
@@ -467,13 +527,16 @@ static int launch_chain1d_t(qw_sim *s, const void *in, void *out, int k, bool dr
     a.rbl_key0 = (unsigned)(s->rbl_seed & 0xffffffffu); a.rbl_key1 = (unsigned)(s->rbl_seed >> 32);
     a.rbl_thr = s->rbl_thr;
     a.t0 = (unsigned)((unsigned long long)s->t & 0xffffffffu);
-    step_chain1d_kernel<R, M, KIND, RBL><<<(unsigned)blocks, WARPS * 32, smem, s->stream>>>(a);
+    a.coins = s->coin_mode == QW_COIN_PER_WALK ? static_cast<const V *>(s->d_coin) : nullptr;
+    a.phases = static_cast<const V *>(s->d_phases);
+    step_chain1d_kernel<R, M, KIND, RBL, FAM><<<(unsigned)blocks, WARPS * 32, smem, s->stream>>>(a);
     QW_LAUNCH_CHECK(s, "step_chain1d_kernel");
     return QW_OK;
 }
 
 template <typename R>
 static int launch_chain1d_r(qw_sim *s, const void *in, void *out, int k, bool dry, double *cost) {
+    if (chain1d_family(s)) return launch_chain1d_t<R, 8, COIN_GENERAL, false, true>(s, in, out, k, dry, cost);
     if (s->rbl) {
         if (s->coin_kind == COIN_HADAMARD) return launch_chain1d_t<R, 16, COIN_HADAMARD, true>(s, in, out, k, dry, cost);
         return launch_chain1d_t<R, 8, COIN_GENERAL, true>(s, in, out, k, dry, cost);
@@ -486,7 +549,8 @@ static int launch_chain1d_r(qw_sim *s, const void *in, void *out, int k, bool dr
 bool chain1d_eligible(const qw_sim *s, int k) {
     const Geom &g = s->g;
     const int M = chain1d_granule(s);
-    return g.dim == 1 && g.boundary == QW_PERIODIC && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
+    const bool plain = s->coin_mode == QW_COIN_UNIFORM && !s->d_phases;
+    return g.dim == 1 && g.boundary == QW_PERIODIC && (plain || (chain1d_family(s) && !s->rbl)) && !s->d_broken &&
            g.en >= 64LL * M && k >= M && k % M == 0 && k <= chain1d_max_k(s);
 }
 

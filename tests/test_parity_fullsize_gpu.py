@@ -255,3 +255,31 @@ def test_k0_is_the_full_config(qw, oracle, dev):
     assert np.max(np.abs(final - psi)) <= 1e-12
     assert np.max(np.abs(P - oracle.probabilities(w.extents, psi))) <= 1e-12
     assert info["sched"] == qw.QW_SCHED_RESIDENT
+
+
+# ------------------------------------------------------------------ a long disordered ring (K4's coin family, 2^24 sites)
+def test_disordered_ring_2_24_sites_through_the_blocked_schedule(qw, oracle, dev):
+    """BASELINE.json:configs[4]'s coin family (an SU(2) coin times per-site phase disorder, eq. 1) on a
+    ring of 2^24 sites, far too long for the resident kernel: AUTO takes the chained blocked kernel; 24 sampled light
+    cones (the seam, chain and tile borders, random sites) against the oracle, which evolves the window with the per-site
+    matrices ph_x * C (R14)."""
+    N, steps = 1 << 24, 96
+    rng = np.random.default_rng(61)
+    c = qi.su2(*rng.uniform(0, 2 * np.pi, 3))
+    ph = np.exp(1j * rng.uniform(0, 2 * np.pi, (1, N)))
+    w = qi.Workload("ring24", 1, (N,), 1, qi.PERIODIC, np.dtype(np.complex128), steps, qi.COIN_UNIFORM, c, phases=ph,
+                    state=qi.random_state(62, 1, N, 2, np.complex128), outputs=("moments",))
+    final, mom, P, info = run_full(qw, w)
+    assert info["sched"] == qw.QW_SCHED_BLOCKED and info["launches"] < steps      # 2 step launches + the output kernels
+    assert abs(mom[0, 0] - 1) <= 1e-12
+    pad = 8
+    half = steps + pad
+    centres = [0, 3, N - 2, N // 2, 256, 255, 14176, 14175, 14176 * 700 + 1] + [int(x) for x in rng.integers(0, N, 15)]
+    worst = 0.0
+    for cx in centres:
+        idx = np.arange(cx - half, cx + half + 1) % N
+        win = np.ascontiguousarray(w.state[0, idx])[None]
+        mats = qi.site_coin_matrices(c[None], ph[:, idx])
+        oracle.step((2 * half + 1,), mats, win, steps, boundary=qi.OPEN, coin_mode=qi.COIN_PER_SITE)
+        worst = max(worst, float(np.max(np.abs(final[0, idx[half - pad:half + pad + 1]] - win[0, half - pad:half + pad + 1]))))
+    assert worst <= 1e-12, worst

@@ -573,6 +573,47 @@ def test_light_cone_diamond_of_the_tiled_kernel(qw, oracle, dev, dtype, coin):
         assert np.array_equal(got, off[0])
 
 
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+def test_coin_family_fast_paths(qw, oracle, dev, dtype):
+    """PAPER.md:35-38 eq. 1 "collections C = (C_v)": per-walk matrices and / or per-site phases on lattices too long for
+    the resident kernel.  The vectorised fused kernel (FAM instance) and, on rings, the chained blocked kernel (phases
+    renamed like a plane that moves one site per step, the entering phase read a step ahead) must give the generic
+    kernel's state bit for bit, and the oracle's within the gates."""
+    rng = np.random.default_rng(51)
+    cases = []
+    for sites, batch, steps, kind in ((40000, 3, 72, "perwalk+ph"), (9001, 2, 40, "perwalk"), (20011, 1, 56, "uniform+ph")):
+        if kind.startswith("perwalk"):
+            a3 = rng.uniform(0, 2 * np.pi, (batch, 3))
+            mode, c = qi.COIN_PER_WALK, qi.su2(a3[:, 0], a3[:, 1], a3[:, 2]).astype(dtype)
+        else:
+            mode, c = qi.COIN_UNIFORM, qi.su2(*rng.uniform(0, 2 * np.pi, 3)).astype(dtype)
+        ph = np.exp(1j * rng.uniform(0, 2 * np.pi, (batch, sites))).astype(dtype) if kind.endswith("+ph") else None
+        cases.append(qi.Workload("fam1d", 1, (sites,), batch, qi.PERIODIC, np.dtype(dtype), steps, mode, c, phases=ph,
+                                 state=qi.random_state(21, batch, sites, 2, dtype, normalise_per_walk=True)))
+    for w in cases:
+        g = gpu_run(qw, w, schedule=qw.QW_SCHED_GENERIC)
+        f = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        assert np.array_equal(g[0], f[0]), w.name
+        for k, max_ctas in ((16, 1), (0, 0)):
+            b = gpu_run(qw, w, schedule=qw.QW_SCHED_BLOCKED, k=k, options={qw.QW_OPT_MAX_CTAS: max_ctas})
+            assert b[3]["sched"] == qw.QW_SCHED_BLOCKED and b[3]["launches"] < g[3]["launches"]
+            assert np.array_equal(g[0], b[0]), (w.sites, k)
+        auto = gpu_run(qw, w)
+        assert auto[3]["sched"] == qw.QW_SCHED_BLOCKED and np.array_equal(auto[0], g[0])
+        check_parity(w, f, oracle_run(oracle, w))
+    # 2D, open and periodic: fused family kernel == generic kernel
+    for boundary in (qi.OPEN, qi.PERIODIC):
+        batch, ext = 2, (97, 130)
+        c = np.stack([qi.random_unitary(rng, 4) for _ in range(batch)]).astype(dtype)
+        ph = np.exp(1j * rng.uniform(0, 2 * np.pi, (batch, ext[0] * ext[1]))).astype(dtype)
+        w = qi.Workload("fam2d", 2, ext, batch, boundary, np.dtype(dtype), 12, qi.COIN_PER_WALK, c, phases=ph,
+                        state=qi.random_state(22, batch, ext[0] * ext[1], 4, dtype, normalise_per_walk=True))
+        g = gpu_run(qw, w, schedule=qw.QW_SCHED_GENERIC)
+        f = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+        assert np.array_equal(g[0], f[0])
+        check_parity(w, f, oracle_run(oracle, w))
+
+
 def test_moments_of_a_narrow_distribution_far_from_the_centre(qw, oracle, dev):
     """qw_moments shifts every block partial to the mean before it forms the second moments: a walker that sits 2^21
     sites from the lattice centre (x^2 ~ 4e12) keeps a variance accurate to 1e-8, where E[x^2] - E[x]^2 in double loses
