@@ -95,7 +95,37 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
     constexpr bool SHARE = FAST && RBL && !DIAG;
     __shared__ unsigned char link_n[SHARE ? U : 1][SHARE ? BS : 1];
     unsigned own[U];
-    if constexpr (SHARE) {
+    if constexpr (SHARE && DIM == 1 && U % 4 == 0) {
+        // 1D: one generator call serves FOUR consecutive sites (reading R27), and for each u the lanes 4q .. 4q+3 of a
+        // warp hold four consecutive sites.  So for every group of four u's, lane l evaluates the call(s) of ONE quad —
+        // row u = ub + (l & 3), quad q = l >> 2 — and the lanes fetch their bit with a shuffle: U/4 calls per thread
+        // instead of U (twice that when the window starts at a site that is not a multiple of 4).
+        const int lane = threadIdx.x & 31;
+        const long long wbase = a.n_lo + (long long)chunk * (BS * U) + (threadIdx.x & ~31);   // site of lane 0 at u = 0
+        const unsigned r = (unsigned)wbase & 3u;                                               // warp-uniform: BS % 4 == 0
+#pragma unroll
+        for (int ub = 0; ub < U; ub += 4) {
+            const unsigned long long x4 = (unsigned long long)(wbase + (long long)(ub + (lane & 3)) * BS + 4 * (lane >> 2));
+            unsigned wd[4];
+            rbl_group_words(x4 >> 2, a.t, (unsigned)w, a.rbl_key0, a.rbl_key1, wd);
+            unsigned bits = 0;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) bits |= ((unsigned long long)wd[i] < a.rbl_thr ? 1u : 0u) << i;
+            if (r != 0) {
+                rbl_group_words((x4 >> 2) + 1, a.t, (unsigned)w, a.rbl_key0, a.rbl_key1, wd);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) bits |= ((unsigned long long)wd[i] < a.rbl_thr ? 1u : 0u) << (4 + i);
+            }
+            const unsigned nibble = (bits >> r) & 0xfu;            // sites x4 .. x4+3
+#pragma unroll
+            for (int du = 0; du < 4; ++du) {
+                const unsigned nib = __shfl_sync(0xffffffffu, nibble, 4 * (lane >> 2) + du);
+                own[ub + du] = (nib >> (lane & 3)) & 1u;
+                link_n[ub + du][threadIdx.x] = (unsigned char)own[ub + du];
+            }
+        }
+        __syncthreads();
+    } else if constexpr (SHARE) {
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             own[u] = 0;

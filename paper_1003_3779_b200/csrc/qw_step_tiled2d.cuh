@@ -35,7 +35,12 @@
 namespace qw {
 
 template <typename R> struct T2dCfg;
-template <> struct T2dCfg<float>  { static constexpr int RM = 4, RN = 2, W = 16; static constexpr bool NSYNC = false; };  // 64 x 64 sites, 128 KiB stage
+#ifndef QW_T2D_F32_RM
+#define QW_T2D_F32_RM 4
+#define QW_T2D_F32_W 16
+#define QW_T2D_F32_NSYNC false
+#endif
+template <> struct T2dCfg<float>  { static constexpr int RM = QW_T2D_F32_RM, RN = 2, W = QW_T2D_F32_W; static constexpr bool NSYNC = QW_T2D_F32_NSYNC; };  // 64 x 64 sites, 128 KiB stage
 #ifndef QW_T2D_F64_RM
 #define QW_T2D_F64_RM 4
 #define QW_T2D_F64_W 8
