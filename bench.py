@@ -414,6 +414,11 @@ def run_gpu(args):
     qw.load()
 
     w = make_workload(args.workload, args.walk_steps)
+    if args.coin == "su2":
+        if w.dim != 1 or w.coin_mode != qi.COIN_UNIFORM:
+            raise SystemExit("--coin su2 needs a 1D workload with a uniform coin")
+        w.coin = qi.su2(0.7, 1.1, 2.3).astype(w.dtype)      # a general 2x2 coin: 16 FP instructions per site-step
+        w.name += "-su2"
     if args.lattice == "diagonal":
         if w.dim != 2:
             raise SystemExit("--lattice diagonal needs a 2D workload")
@@ -668,6 +673,7 @@ def main():
     ap.add_argument("--k", type=int, default=0)
     ap.add_argument("--no-window", action="store_true")
     ap.add_argument("--lattice", default=None, choices=["natural", "diagonal"], help="override the 2D lattice kind")
+    ap.add_argument("--coin", default=None, choices=["su2"], help="k1 / k1c64 only: a general SU(2) coin instead of Hadamard")
     ap.add_argument("--rbl", type=float, default=None, help="random broken links redrawn every step with this probability")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="qw_set_option(key, value) by number, e.g. --opt 1=1 forces the halo kernel of the blocked 1D schedule")

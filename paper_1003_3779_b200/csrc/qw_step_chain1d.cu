@@ -131,14 +131,14 @@ __device__ __forceinline__ void chain1d_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M],
     for (int q = 0; q < M; ++q) {
         const int p = (q + 2 * U) % M;
         cplx<R> v[2] = {Rp[q], Lp[p]};
-        if constexpr (KIND == COIN_HADAMARD && M == 16) {
-            // deferred scale, as in qw_step_blocked1d.cu: M-1 bare butterflies, then one scaled step with s^M
-            if constexpr (U + 1 < M) {
+        if constexpr (KIND == COIN_HADAMARD && M % 16 == 0) {
+            // deferred scale, as in qw_step_blocked1d.cu: 15 bare butterflies, then one scaled step with s^16
+            if constexpr (U % 16 != 15) {
                 const cplx<R> r = v[0], l = v[1];
                 v[0] = cx_add(r, l);
                 v[1] = cx_sub(r, l);
             } else {
-                apply_coin<R, 2, COIN_HADAMARD>(C + 1, v);      // C[1] = s^M
+                apply_coin<R, 2, COIN_HADAMARD>(C + 1, v);      // C[1] = s^16
             }
         } else {
             apply_coin<R, 2, KIND>(C, v);
@@ -259,6 +259,9 @@ template <int M, int ES> __device__ __forceinline__ int chain_pos(int row, int c
 
 template <typename R, int M> struct Chain1dShape {
     // warps per CTA x CTAs per SM: complex128 8 warps per SM, complex64 12 (measured: 16 warps at 128 registers are slower)
+#ifndef QW_CHAIN_M32
+#define QW_CHAIN_M32 0      // 32 sites per lane for complex64 (8 warps per SM at 236 registers): measured 5.5e12 against 6.3e12 on K1
+#endif
 #ifndef QW_CHAIN_WARPS
 #define QW_CHAIN_WARPS 4
 #endif
@@ -269,7 +272,7 @@ template <typename R, int M> struct Chain1dShape {
 #define QW_CHAIN_MINB32 3
 #endif
     static constexpr int WARPS = QW_CHAIN_WARPS;
-    static constexpr int MINB = sizeof(R) == 8 ? QW_CHAIN_MINB64 : QW_CHAIN_MINB32;
+    static constexpr int MINB = (sizeof(R) == 8 || M == 32) ? QW_CHAIN_MINB64 : QW_CHAIN_MINB32;
     // shared memory of one warp, in elements: two prefetched input planes, HALF a plane of output staging, exchange
     static constexpr int SMEM_ELEMS = 2 * 32 * M + 16 * M +
         (Chain1dExchange<R>::SMEM ? 2 * Chain1dExchange<R>::AREA : 4 * Chain1dExchange<R>::KMAX);
@@ -294,7 +297,7 @@ step_chain1d_kernel(const Chain1dArgs<R> a) {
     R C[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) C[i] = a.coin[i];
-    if constexpr (KIND == COIN_HADAMARD && M == 16) C[1] = a.scale_m;           // the (zero) imaginary part of C[0][0] is unused
+    if constexpr (KIND == COIN_HADAMARD && M % 16 == 0) C[1] = a.scale_m;           // the (zero) imaginary part of C[0][0] is unused
 
     // element i*32 + lane of a tile: row (i*32 + lane) / M, col (i*32 + lane) % M
     int pos_co[M];                                                              // coalesced-side staging positions
@@ -520,7 +523,7 @@ static int launch_chain1d_t(qw_sim *s, const void *in, void *out, int k, bool dr
     a.k = k;
     for (int i = 0; i < 8; ++i) a.coin[i] = (R)s->h_coin[i];
     R sm = (R)1;
-    for (int i = 0; i < M; ++i) sm = (R)(sm * a.coin[0]);    // s^M by repeated rounded products in the handle's precision
+    for (int i = 0; i < 16; ++i) sm = (R)(sm * a.coin[0]);   // s^16 by repeated rounded products in the handle's precision
     a.scale_m = sm;
     long long blocks = (a.total_chains + WARPS - 1) / WARPS;
     if (blocks > grid_warps / WARPS) blocks = grid_warps / WARPS;
@@ -541,7 +544,14 @@ static int launch_chain1d_r(qw_sim *s, const void *in, void *out, int k, bool dr
         if (s->coin_kind == COIN_HADAMARD) return launch_chain1d_t<R, 16, COIN_HADAMARD, true>(s, in, out, k, dry, cost);
         return launch_chain1d_t<R, 8, COIN_GENERAL, true>(s, in, out, k, dry, cost);
     }
-    if (s->coin_kind == COIN_HADAMARD) return launch_chain1d_t<R, 16, COIN_HADAMARD, false>(s, in, out, k, dry, cost);
+    if (s->coin_kind == COIN_HADAMARD) {
+        // complex64: 32 sites per lane when the depth allows it (the register file holds twice as many complex64 sites;
+        // half as many lane crossings and tile stagings per site)
+        if constexpr (sizeof(R) == 4 && QW_CHAIN_M32) {
+            if (k % 32 == 0 && s->g.en >= 64LL * 32) return launch_chain1d_t<R, 32, COIN_HADAMARD, false>(s, in, out, k, dry, cost);
+        }
+        return launch_chain1d_t<R, 16, COIN_HADAMARD, false>(s, in, out, k, dry, cost);
+    }
     return launch_chain1d_t<R, 8, COIN_GENERAL, false>(s, in, out, k, dry, cost);
 }
 
