@@ -41,7 +41,8 @@
  * Errors: every call returns QW_OK (0) or a negative code, never throws or aborts; after an
  * error the handle is unchanged (except QW_ECUDA raised by an asynchronous failure).
  * qw_last_error() returns a thread-local message for the last non-zero return.
- * A handle must not be used from two host threads at the same time.
+ * A handle must not be used from two host threads at the same time.  A handle belongs to the CUDA device that was
+ * current when it was created; calls that touch its state return QW_EINVAL while another device is current.
  */
 #ifndef QW_H_
 #define QW_H_

@@ -100,6 +100,17 @@ static int stream_state(qw_sim *s, void *host, bool to_device) {
     return QW_OK;
 }
 
+// Every call that touches device state must run with the handle's device current: kernels are launched on the current
+// device with the handle's pointers, so a mismatch would be a sticky context error instead of a return code.
+static int check_device(const qw_sim *s) {
+    int dev = -1;
+    QW_CUDA(cudaGetDevice(&dev));
+    if (dev != s->device)
+        return fail(QW_EINVAL, "the handle lives on device %d but device %d is current (cudaSetDevice first)", s->device, dev);
+    return QW_OK;
+}
+#define QW_ON_DEVICE(s) do { int qw_rc_ = check_device(s); if (qw_rc_) return qw_rc_; } while (0)
+
 static int classify_coin(const double *C, int cdim, int dtype) {
     auto re = [&](int a, int b) { return C[2 * (a * cdim + b)]; };
     auto im = [&](int a, int b) { return C[2 * (a * cdim + b) + 1]; };
@@ -259,6 +270,7 @@ int qw_destroy(qw_sim *s) {
 int qw_set_stream(qw_sim *s, void *cuda_stream) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     QW_CUDA(cudaStreamSynchronize(s->stream));   // keep work already issued ordered before the switch
     s->stream = static_cast<cudaStream_t>(cuda_stream);
     return QW_OK;
@@ -280,6 +292,7 @@ int qw_set_lattice(qw_sim *s, int lattice) {
 int qw_set_coin(qw_sim *s, int mode, const void *coin) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     if (!coin) return fail(QW_EINVAL, "coin is NULL");
     if (mode != QW_COIN_UNIFORM && mode != QW_COIN_PER_WALK && mode != QW_COIN_PER_SITE)
         return fail(QW_EINVAL, "unknown coin mode %d", mode);
@@ -317,6 +330,7 @@ int qw_set_coin(qw_sim *s, int mode, const void *coin) {
 int qw_set_site_phases(qw_sim *s, const void *phases) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     QW_CUDA(cudaStreamSynchronize(s->stream));
     if (!phases) { if (s->d_phases) cudaFree(s->d_phases); s->d_phases = nullptr; return QW_OK; }
     const size_t bytes = (size_t)s->g.batch * (size_t)s->g.sites * s->esize;
@@ -333,6 +347,7 @@ int qw_set_site_phases(qw_sim *s, const void *phases) {
 int qw_set_broken_links(qw_sim *s, const uint8_t *mask) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     QW_CUDA(cudaStreamSynchronize(s->stream));
     if (!mask) { if (s->d_broken) cudaFree(s->d_broken); s->d_broken = nullptr; return QW_OK; }
     const size_t bytes = (size_t)s->g.batch * (size_t)s->g.sites * (size_t)s->g.cdim;
@@ -360,6 +375,7 @@ int qw_set_random_broken_links(qw_sim *s, int enable, double p, uint64_t seed) {
 int qw_set_state(qw_sim *s, const void *amps) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     if (!amps) return fail(QW_EINVAL, "amps is NULL");
     const Geom &g = s->g;
     const size_t bytes = (size_t)g.batch * (size_t)g.sites * (size_t)g.cdim * s->esize;
@@ -376,6 +392,7 @@ int qw_set_state(qw_sim *s, const void *amps) {
 int qw_set_state_delta(qw_sim *s, const int64_t *site, const void *coin_vec) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     if (!site || !coin_vec) return fail(QW_EINVAL, "site or coin_vec is NULL");
     const Geom &g = s->g;
     long long st[2] = {0, 0};
@@ -410,6 +427,7 @@ int qw_get_state(const qw_sim *cs, void *amps) {
     clear_error();
     qw_sim *s = const_cast<qw_sim *>(cs);
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     if (!amps) return fail(QW_EINVAL, "amps is NULL");
     if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
     const Geom &g = s->g;
@@ -422,6 +440,7 @@ int qw_get_state(const qw_sim *cs, void *amps) {
 int qw_step(qw_sim *s, int64_t n) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     if (n < 0) return fail(QW_EINVAL, "n must be >= 0 (got %lld)", (long long)n);
     if (!s->has_coin) return fail(QW_ESTATE, "qw_step before qw_set_coin");
     if (!s->has_state) return fail(QW_ESTATE, "qw_step before qw_set_state");
@@ -535,6 +554,7 @@ int qw_step(qw_sim *s, int64_t n) {
 int qw_step_inverse(qw_sim *s, int64_t n) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     if (n < 0) return fail(QW_EINVAL, "n must be >= 0 (got %lld)", (long long)n);
     if (!s->has_coin) return fail(QW_ESTATE, "qw_step_inverse before qw_set_coin");
     if (!s->has_state) return fail(QW_ESTATE, "qw_step_inverse before qw_set_state");
@@ -553,6 +573,7 @@ int qw_probabilities(const qw_sim *cs, void *out) {
     clear_error();
     qw_sim *s = const_cast<qw_sim *>(cs);
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     if (!out) return fail(QW_EINVAL, "out is NULL");
     if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
     const size_t bytes = (size_t)s->g.batch * (size_t)s->g.sites * (s->esize / 2);
@@ -570,6 +591,7 @@ int qw_moments(const qw_sim *cs, double *out) {
     clear_error();
     qw_sim *s = const_cast<qw_sim *>(cs);
     if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
     if (!out) return fail(QW_EINVAL, "out is NULL");
     if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
     const size_t bytes = (size_t)s->g.batch * (s->g.dim == 1 ? 3 : 6) * sizeof(double);
