@@ -39,3 +39,22 @@ def test_paper_table_context_workloads():
     cfg = bench.workload_config("t2", t2)
     assert "DIAGONAL" in cfg["workload"] and cfg["baseline_config"] is None
     assert bench.workload_config("k1", qi.k1(sites=64, steps=3))["baseline_config"] == 1
+
+
+def test_gpus_n_outside_torchrun_starts_its_own_ranks():
+    """`python bench.py --gpus 2` with no WORLD_SIZE in the environment re-executes itself under torch.distributed.run with
+    two ranks (it used to time one replica and print n_gpus 1).  Checked with the reference arm, which needs
+    no GPU: rank 0 prints the one JSON line, rank 1 exits 0 without work."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                        "--warmup", "0", "--workload", "k0"], capture_output=True, text=True, timeout=600, env=env, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
