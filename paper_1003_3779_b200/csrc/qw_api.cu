@@ -524,7 +524,8 @@ int qw_step(qw_sim *s, int64_t n) {
         s->last_k = chain ? kchain : kmax;
         // multiples of M with the big tiles, then a remainder of 4 .. 15 steps with short 8- / 4-step launches (small
         // tiles, the fused kernel's arithmetic), then at most 3 fused single steps
-        while (remaining >= (halo ? 4 : M)) {
+        // (neither kernel applies — e.g. random broken links with a user depth below the tile granule: all steps run fused)
+        while ((halo || chain) && remaining >= (halo ? 4 : M)) {
             int rc;
             int kk;
             if (chain && remaining >= M) {

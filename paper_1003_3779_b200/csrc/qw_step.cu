@@ -126,10 +126,36 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
         }
         __syncthreads();
     } else if constexpr (SHARE) {
+        // 2D, even row length and an even first column (the launcher extends the box by one site if needed): the lanes
+        // 2q, 2q+1 hold the two sites of one generator group, so the EVEN lane evaluates the call of the pair's own links
+        // and the ODD lane the call of the pair's upper-row links (owners (m-1, n), (m-1, n+1): numbers 2o'+1, 2o'+3 of
+        // group o'/2); two shuffles hand the bits out.  One call per site instead of two.
+        const bool coop = DIM == 2 && ((a.en & 1) == 0) && ((a.n_lo & 1) == 0);
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             own[u] = 0;
-            if (live[u]) {
+            if (coop) {
+                const int lane = threadIdx.x & 31;
+                const long long nl = a.n_lo + n_base + (long long)u * BS;            // parity of nl = parity of the lane
+                unsigned long long grp;
+                if ((lane & 1) == 0) {
+                    grp = (unsigned long long)(m * a.en + nl) >> 1;
+                } else {
+                    long long mu = m - 1;
+                    if (mu < 0) mu += a.em;
+                    grp = (unsigned long long)(mu * a.en + nl - 1) >> 1;
+                }
+                unsigned wd[4];
+                rbl_group_words(grp, a.t, (unsigned)w, a.rbl_key0, a.rbl_key1, wd);
+                unsigned pack = 0;
+#pragma unroll
+                for (int i = 0; i < 4; ++i) pack |= ((unsigned long long)wd[i] < a.rbl_thr ? 1u : 0u) << i;
+                const unsigned ownpack = __shfl_sync(0xffffffffu, pack, lane & ~1);
+                const unsigned uppack = __shfl_sync(0xffffffffu, pack, lane | 1);
+                const unsigned mine = (lane & 1) ? (ownpack >> 2) & 3u : ownpack & 3u;   // bit 0: own n-link, bit 1: own m-link
+                const unsigned up = (lane & 1) ? (uppack >> 3) & 1u : (uppack >> 1) & 1u; // words 3 / 1: the upper row's m-links
+                own[u] = mine | (up << 2) | 8u;
+            } else if (live[u]) {
                 // the links this site owns: numbers owner * DIM + axis (1D: word owner & 3 of call owner / 4; 2D: words
                 // 2 (owner & 1) + axis of call owner / 2)
                 const unsigned long long owner = (unsigned long long)(m * a.en + a.n_lo + n_base + (long long)u * BS);
@@ -215,7 +241,8 @@ step_scatter_kernel(const StepArgs<R, 2 * DIM> a) {
                         if (threadIdx.x > 0) broken = link_n[u][threadIdx.x - 1] != 0;
                         else if (u > 0) broken = link_n[u > 0 ? u - 1 : 0][BS - 1] != 0;
                         else broken = rbl_link_broken<DIM>(a, w, m, n, tm, tn, dm, dn);         // first site of the block
-                    } else broken = rbl_link_broken<DIM>(a, w, m, n, tm, tn, dm, dn);           // the upper row's link
+                    } else broken = (own[u] & 8u) ? (own[u] & 4u) != 0                          // the upper row's link
+                                                  : rbl_link_broken<DIM>(a, w, m, n, tm, tn, dm, dn);
                     if (broken) stay = true;
                 }
             } else if constexpr (RBL) {
@@ -334,6 +361,9 @@ static int launch_step_t(qw_sim *s, const void *in, void *out, const Box &box, b
     StepArgs<R, 2 * DIM> a;
     fill_args<R, DIM>(s, in, out, box, a);
     const bool fast = allow_fast && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken;
+    if (fast && s->rbl && DIM == 2 && s->g.lattice == QW_NATURAL && (s->g.en & 1) == 0 && (a.n_lo & 1)) {
+        a.n_lo -= 1; a.box_n += 1;      // even first column: lane pairs = generator groups (the extra site is a zero of the window)
+    }
     // coin families on the vectorised path: per-walk matrices and / or site phases (natural lattice, no links)
     const bool fam = allow_fast && !fast && s->coin_mode != QW_COIN_PER_SITE && !s->d_broken && !s->rbl &&
                      s->g.lattice == QW_NATURAL;

@@ -303,7 +303,7 @@ def test_chained_blocked_1d_kernel(qw, oracle, dev, dtype, coin):
     rng = np.random.default_rng(23)
     M = 16 if coin == "hadamard" else 8
     cases = ((20000, 112, 48, 1, 1), (3001, 64, 16, 3, 2), (70001, 131, 0, 1, 0), (64 * M, 64, 64, 2, 1),
-             (100003, 200, 64, 1, 3), (9973, 40, 32, 2, 1))
+             (100003, 200, 64, 1, 3), (9973, 40, 32, 2, 1), (2048, 48, 16, 20, 1))     # last: 20 chains over 4 warps
     for sites, steps, k, batch, max_ctas in cases:
         c = qi.hadamard(dtype) if coin == "hadamard" else qi.su2(*rng.uniform(0, 2 * np.pi, 3)).astype(dtype)
         w = qi.Workload("chain", 1, (sites,), batch, qi.PERIODIC, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,

@@ -169,5 +169,25 @@ def test_rbl_inside_the_temporally_blocked_ring_kernel(qw, oracle, dev, dtype, c
         assert np.array_equal(b, s2)
         if dtype == np.complex128:
             assert np.max(np.abs(mom[:, 0] - 1)) < 1e-12
+    low = gpu_rbl(qw, w, p, SEED, steps, schedule=qw.QW_SCHED_BLOCKED, k=4)   # depth below the tile granule: fused steps
+    assert np.array_equal(low[0], f)
     auto = gpu_rbl(qw, w, p, SEED, steps)                             # AUTO takes the blocked kernel on a long ring
     assert auto[2] == qw.QW_SCHED_BLOCKED and np.array_equal(auto[0], b)
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+def test_rbl_2d_even_rows_share_generator_calls_between_lane_pairs(qw, oracle, dev, dtype, boundary):
+    """2D natural lattice with an even row length: the fused-RBL kernel lets lane pairs share one generator call for the
+    pair's own links and one for its upper-row links.  Delta start with the light-cone window at odd and even first
+    columns (the launcher extends the box to an even column), several CTAs per row, rows that wrap to the last row."""
+    c = qi.dft4(dtype)
+    dc = np.array([0.5, -0.5, -0.5, 0.5], dtype=dtype)
+    for ext, site, steps in (((60, 64), (30, 31), 25), ((9, 1200), (0, 600), 40), ((34, 530), (33, 2), 30)):
+        w = qi.Workload("rbl2d", 2, ext, 2, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c, delta_site=site, delta_coin=dc)
+        psi = oracle_rbl(oracle, w, 0.2, SEED, steps)
+        on = gpu_rbl(qw, w, 0.2, SEED, steps, schedule=qw.QW_SCHED_FUSED, window=True)
+        off = gpu_rbl(qw, w, 0.2, SEED, steps, schedule=qw.QW_SCHED_FUSED, window=False)
+        gen = gpu_rbl(qw, w, 0.2, SEED, steps, schedule=qw.QW_SCHED_GENERIC, window=False)
+        assert np.array_equal(on[0], off[0]) and np.array_equal(off[0], gen[0]), (ext, site)
+        close(w, on[0], psi)
