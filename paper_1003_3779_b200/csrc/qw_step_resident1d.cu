@@ -26,6 +26,8 @@ struct Resident1dArgs {
     typename Cx<R>::T *out;
     long long n_sites, walk_stride, plane_stride;
     long long n_steps;
+    long long x_off;                   // first site of thread 0: the CTA covers [x_off, x_off + threads * M) (a stage of the
+                                       // light cone, see launch_resident_shape); everything outside is exactly zero
     const typename Cx<R>::T *coins;    // per-walk matrices or nullptr (uniform)
     const typename Cx<R>::T *phases;   // [walk][site] or nullptr
     int window;                        // 1: skip warps outside the light cone
@@ -35,7 +37,8 @@ struct Resident1dArgs {
 
 template <typename R>
 struct ResidentCtx {
-    typename Cx<R>::T *edgeR, *edgeL, *wrapR, *wrapL;   // [2][nw], [2][nw], [2], [2]
+    typename Cx<R>::T *xR, *xL, *wrapR, *wrapL;         // exchange rows [2][T + 2] each (T = threads), wrap slots [2], [2]
+    int xstride;                                        // T + 2
     const typename Cx<R>::T *ph;                        // padded per-site phases of this walk (shared)
     int lane, wid, nw, tid;
     bool lo_thread;        // owns site 0
@@ -94,23 +97,21 @@ __device__ __forceinline__ void resident_step(cplx<R> (&Rp)[M], cplx<R> (&Lp)[M]
         for (int i = 0; i < M; ++i)
             if (i == cx.hi_index) hiR = Rp[(i - U + M) % M];
     }
-    cplx<R> inR = shfl_up_cx(outR), inL = shfl_down_cx(outL);
+    // The element per plane that leaves the thread goes through a shared-memory row (thread t writes entry t + 1, reads
+    // entry t of the R row and entry t + 2 of the L row; entries 0 and T + 1 are zeros: beyond the CTA's range there is
+    // nothing): two stores, the step's barrier, two loads — no shuffles, no special case at warp boundaries.  (An FP64
+    // instruction holds the issue port for two cycles, so the 8 SHFL + ~12 register moves this replaces were paid in FP64 time.)
     const int par = (int)(s & 1);
-    if (cx.nw > 1) {
-        if (cx.lane == 31) cx.edgeR[par * cx.nw + cx.wid] = to_v<R>(outR);
-        if (cx.lane == 0) cx.edgeL[par * cx.nw + cx.wid] = to_v<R>(outL);
-    }
+    typename Cx<R>::T *xr = cx.xR + par * cx.xstride + cx.tid, *xl = cx.xL + par * cx.xstride + cx.tid;
+    xr[1] = to_v<R>(outR);
+    xl[1] = to_v<R>(outL);
     if constexpr (!OPEN) {
         if (cx.hi_index >= 0) cx.wrapR[par] = to_v<R>(hiR);
         if (cx.lo_thread) cx.wrapL[par] = to_v<R>(outL);
     }
     if (cx.nw > 1) __syncthreads(); else __syncwarp();
-    if (cx.nw > 1) {
-        if (cx.lane == 0 && cx.wid > 0) inR = from_v<R>(cx.edgeR[par * cx.nw + cx.wid - 1]);
-        if (cx.lane == 31 && cx.wid < cx.nw - 1) inL = from_v<R>(cx.edgeL[par * cx.nw + cx.wid + 1]);
-    }
-    Rp[QS] = inR;
-    Lp[PS] = inL;
+    Rp[QS] = from_v<R>(xr[0]);
+    Lp[PS] = from_v<R>(xl[2]);
     // site 0 and site N-1: reflecting walls (RBL = 0) or the periodic seam
     if (cx.lo_thread) Rp[QS] = OPEN ? outL : from_v<R>(cx.wrapR[par]);
     if (cx.hi_warp) {
@@ -141,22 +142,31 @@ step_resident1d_kernel(const Resident1dArgs<R> a) {
     const long long w = blockIdx.x, N = a.n_sites;
     V *sm = reinterpret_cast<V *>(smem_raw);
     ResidentCtx<R> cx;
-    cx.edgeR = sm; cx.edgeL = sm + 2 * nw; cx.wrapR = sm + 4 * nw; cx.wrapL = sm + 4 * nw + 2;
-    V *ph = sm + 4 * nw + 4;
+    const int T = blockDim.x;
+    cx.xstride = T + 2;
+    cx.xR = sm; cx.xL = sm + 2 * (T + 2); cx.wrapR = sm + 4 * (T + 2); cx.wrapL = sm + 4 * (T + 2) + 2;
+    V *ph = sm + 4 * (T + 2) + 4;
+    if (tid < 2) {                                  // the zero entries beyond both ends of the exchange rows
+        V z; z.x = 0; z.y = 0;
+        for (int par = 0; par < 2; ++par) {
+            cx.xR[par * (T + 2) + tid * (T + 1)] = z;
+            cx.xL[par * (T + 2) + tid * (T + 1)] = z;
+        }
+    }
     cx.ph = ph;
     cx.tid = tid; cx.lane = tid & 31; cx.wid = tid >> 5; cx.nw = nw;
-    const long long x0 = (long long)tid * M;
-    cx.lo_thread = (tid == 0);
+    const long long x0 = a.x_off + (long long)tid * M;
+    cx.lo_thread = (tid == 0) && a.x_off == 0;
     cx.hi_index = (N - 1 >= x0 && N - 1 < x0 + M) ? (int)(N - 1 - x0) : -1;
     cx.hi_warp = __any_sync(0xffffffffu, cx.hi_index >= 0);
-    cx.warp_lo = (long long)cx.wid * 32 * M;
+    cx.warp_lo = a.x_off + (long long)cx.wid * 32 * M;
     cx.warp_hi = cx.warp_lo + 32 * M - 1;
     cx.window = a.window; cx.centre = a.centre; cx.radius0 = a.radius0;
 
     if constexpr (PHASES) {
         for (long long e = tid; e < (long long)blockDim.x * M; e += blockDim.x) {
             V z; z.x = 0; z.y = 0;
-            if (e < N) z = a.phases[w * N + e];
+            if (a.x_off + e < N) z = a.phases[w * N + a.x_off + e];
             ph[(e / M) * (M | 1) + (e % M)] = z;       // odd row length: conflict-free 16-byte reads
         }
     }
@@ -209,24 +219,22 @@ bool resident1d_eligible(const qw_sim *s) {
            g.batch <= 0x7fffffffLL;
 }
 
+// One launch = all walks advanced `steps` steps by CTAs of `threads` threads that cover the sites [x_off, x_off + threads*M).
 template <typename R, int M, int KIND, bool PHASES, int MAXT, int MINB>
-static int launch_resident_shape(qw_sim *s, const void *in, void *out, long long n) {
+static int launch_resident_stage(qw_sim *s, const void *in, void *out, long long steps, long long x_off, int threads,
+                                 long long radius0, bool cone_ok) {
     typedef typename Cx<R>::T V;
     const Geom &g = s->g;
     Resident1dArgs<R> a;
     a.in = static_cast<const V *>(in); a.out = static_cast<V *>(out);
-    a.n_sites = g.en; a.walk_stride = g.walk_stride; a.plane_stride = g.plane_stride; a.n_steps = n;
+    a.n_sites = g.en; a.walk_stride = g.walk_stride; a.plane_stride = g.plane_stride; a.n_steps = steps;
+    a.x_off = x_off;
     a.coins = s->coin_mode == QW_COIN_PER_WALK ? static_cast<const V *>(s->d_coin) : nullptr;
     a.phases = static_cast<const V *>(s->d_phases);
-    // the cone test is only meaningful while the cone has not wrapped around a periodic lattice
-    const bool cone_ok = s->window_enabled && s->window_valid &&
-                         (g.boundary == QW_OPEN || (s->centre[0] - (s->radius + n + 1) >= 0 && s->centre[0] + (s->radius + n + 1) < g.en));
-    a.window = cone_ok ? 1 : 0; a.centre = s->centre[0]; a.radius0 = s->radius;
+    a.window = cone_ok ? 1 : 0; a.centre = s->centre[0]; a.radius0 = radius0;
     for (int i = 0; i < 8; ++i) a.coin[i] = (R)s->h_coin[i];
-    int threads = (int)((g.en + M - 1) / M);
-    threads = (threads + 31) / 32 * 32;
     const int nw = threads / 32;
-    const size_t smem = sizeof(V) * (size_t)(4 * nw + 4 + (PHASES ? (size_t)threads * (M | 1) : 0));
+    const size_t smem = sizeof(V) * (size_t)(4 * (threads + 2) + 4 + (PHASES ? (size_t)threads * (M | 1) : 0));
     auto launch = [&](auto kernel) -> int {
         if (smem > 48 * 1024)
             QW_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -239,15 +247,73 @@ static int launch_resident_shape(qw_sim *s, const void *in, void *out, long long
     QW_LAUNCH_CHECK(s, "step_resident1d_kernel");
     {   // site-steps actually computed: the warps the per-step cone test of the kernel leaves active
         double touched = 0.0;
-        for (long long st = 0; st < n; ++st) {
-            if (!a.window) { touched += (double)g.en; continue; }
-            const long long r = a.radius0 + st + 1;
+        for (long long st = 0; st < steps; ++st) {
+            const long long r = radius0 + st + 1;
             for (int wi = 0; wi < nw; ++wi) {
-                const long long lo = (long long)wi * 32 * M, hi = lo + 32 * M - 1;
-                if (lo <= a.centre + r && hi >= a.centre - r) touched += (double)((hi < g.en ? hi : g.en - 1) - lo + 1);
+                const long long lo = x_off + (long long)wi * 32 * M, hi = lo + 32 * M - 1;
+                if (lo >= g.en) break;
+                if (!a.window || (lo <= a.centre + r && hi >= a.centre - r)) touched += (double)((hi < g.en ? hi : g.en - 1) - lo + 1);
             }
         }
         s->touched += touched * (double)g.batch;
+    }
+    return QW_OK;
+}
+
+// n steps of all walks.  With a known light cone (after a delta start the walker is within t sites of its
+// origin) the first steps need only the few warps around the origin: the run is cut into STAGES whose CTAs cover 2, 4, 8, ...
+// warps' worth of sites around the cone (everything outside is exactly zero in both buffers) — small CTAs, many per SM —
+// until the cone needs the whole walk.  A stage ends when the cone (+ M + 1 sites of margin, so that the end threads of the
+// CTA hold nothing but zeros and need no boundary code) would leave its range; ranges are clamped to the lattice, a clamped
+// side is a real wall.  Without a cone: one launch over the whole walk.
+template <typename R, int M, int KIND, bool PHASES, int MAXT, int MINB>
+static int launch_resident_shape(qw_sim *s, const void *in, void *out, long long n) {
+    const Geom &g = s->g;
+    int full_threads = (int)((g.en + M - 1) / M);
+    full_threads = (full_threads + 31) / 32 * 32;
+    // the cone test is only meaningful while the cone has not wrapped around a periodic lattice
+    const bool cone_ok = s->window_enabled && s->window_valid &&
+                         (g.boundary == QW_OPEN || (s->centre[0] - (s->radius + n + 1) >= 0 && s->centre[0] + (s->radius + n + 1) < g.en));
+    struct Stage { long long steps, x_off; int threads; };
+    Stage plan[12];
+    int np = 0;
+    long long done = 0, radius = s->radius;
+    // (staging pays when there are enough walks to fill the machine with small CTAs; a single walk is latency bound)
+    if (cone_ok && g.batch >= s->sm_count) {
+        static const int widths[] = {2, 3, 4, 6, 8, 10, 12, 16, 24};
+        for (int wi = 0; wi < 9 && np < 10 && done < n; ++wi) {
+            const int nw = widths[wi];
+            if (nw * 32 >= full_threads) break;
+            const long long S = (long long)nw * 32 * M;
+            long long lo = s->centre[0] - S / 2;
+            if (lo < 0) lo = 0;
+            if (lo + S > g.en) lo = g.en - S;
+            if (lo < 0) break;
+            lo = lo / 2 * 2;                                           // 16-byte aligned complex64 rows stay aligned
+            // steps this range can hold: after t steps the support is within radius + t (+1 of pad) of the centre
+            long long tmax = n - done;
+            if (lo > 0) { const long long t = (s->centre[0] - lo) - (M + 1) - (radius + 1); if (t < tmax) tmax = t; }
+            if (lo + S < g.en) { const long long t = (lo + S - 1 - s->centre[0]) - (M + 1) - (radius + 1); if (t < tmax) tmax = t; }
+            if (tmax < 16) continue;
+            plan[np++] = Stage{tmax, lo, nw * 32};
+            done += tmax; radius += tmax;
+        }
+    }
+    if (done < n) plan[np++] = Stage{n - done, 0, full_threads};
+    if (np % 2 == 0) {       // an even number of launches would end in the input buffer: fold the first stage into the second
+        plan[1].steps += plan[0].steps;
+        for (int i = 0; i + 1 < np; ++i) plan[i] = plan[i + 1];
+        --np;
+    }
+    const void *src = in;
+    void *dst = out;
+    radius = s->radius;
+    for (int i = 0; i < np; ++i) {
+        int rc = launch_resident_stage<R, M, KIND, PHASES, MAXT, MINB>(s, src, dst, plan[i].steps, plan[i].x_off, plan[i].threads,
+                                                                      radius, cone_ok);
+        if (rc) return rc;
+        radius += plan[i].steps;
+        const void *t = src; src = dst; dst = const_cast<void *>(t);
     }
     return QW_OK;
 }
