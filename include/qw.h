@@ -73,10 +73,13 @@ enum {
                               on a ring chained through the stream of L amplitudes, no halo recomputation;
                               2D: shared-memory tiles loaded by TMA)                                    */
     QW_SCHED_RESIDENT = 4, /* one CTA per walk, state on the SM for all n steps                         */
-    QW_SCHED_TILED = 5     /* 2D temporally blocked, tiles held in REGISTERS by persistent CTAs with TMA
-                              prefetch; k in {2, 4, 6, 8}; honours the light-cone window.  Natural lattice:
-                              any boundary.  Diagonal lattice: torus, or open lattice after
-                              qw_set_state_delta (the fused kernel takes over when the cone reaches a wall) */
+    QW_SCHED_TILED = 5     /* 2D temporally blocked with the state of k steps held in REGISTERS; honours the
+                              light-cone window.  Natural lattice, any boundary: every warp streams down a strip
+                              of columns with a k-level pipeline of rows in its registers (no halo along m, no
+                              barriers; k even, <= 12 for complex64, <= 8 for complex128), or — QW_OPT_TILED2D_KERNEL
+                              — tiles held by persistent CTAs with TMA prefetch (k in {2, 4, 6, 8}).  Diagonal
+                              lattice (tiles only): torus, or open lattice after qw_set_state_delta (the fused
+                              kernel takes over when the cone reaches a wall)                                  */
 };
 
 /* qw_get_info keys */
@@ -97,10 +100,13 @@ enum {
     QW_OPT_MAX_CTAS = 0,        /* cap on the grid of the persistent (blocked 1D) kernels; 0 = one grid
                                    that fills every SM (default).  For sharing a GPU and for tests that want
                                    long per-warp tile chains on small lattices; results do not depend on it */
-    QW_OPT_BLOCKED1D_KERNEL = 1 /* which temporally blocked 1D kernel QW_SCHED_BLOCKED uses on a ring: 0 = the
+    QW_OPT_BLOCKED1D_KERNEL = 1,/* which temporally blocked 1D kernel QW_SCHED_BLOCKED uses on a ring: 0 = the
                                    cheaper one (default), 1 = warp tiles with recomputed halos, 2 = chained
                                    tiles (no halo work; rings with a uniform coin, else falls back to 1).
                                    Both execute the same arithmetic per site: bit-identical results          */
+    QW_OPT_TILED2D_KERNEL = 2   /* which register-resident 2D kernel QW_SCHED_TILED uses on the natural lattice:
+                                   0 = the streaming kernel (default), 1 = CTA tiles with TMA prefetch,
+                                   2 = the streaming kernel.  Bit-identical results                         */
 };
 
 /* Create a walk on a dim-dimensional lattice (dim = 1 or 2) with `extents[d] >= 1` sites per
@@ -180,7 +186,7 @@ int qw_probabilities(const qw_sim *s, void *out);
 int qw_moments(const qw_sim *s, double *out);
 
 /* Force a schedule (QW_SCHED_*); k = temporal block depth for QW_SCHED_BLOCKED / QW_SCHED_TILED
- * (0 = library default; QW_SCHED_TILED accepts 2, 4, 6 or 8, else QW_EINVAL).
+ * (0 = library default; QW_SCHED_TILED accepts the even depths listed at QW_SCHED_TILED, else QW_EINVAL).
  * QW_EUNSUPPORTED if the handle's configuration has no such kernel. */
 int qw_set_schedule(qw_sim *s, int schedule, int k);
 

@@ -23,7 +23,7 @@ QW_COIN_UNIFORM, QW_COIN_PER_WALK, QW_COIN_PER_SITE = 0, 1, 2
 QW_SCHED_AUTO, QW_SCHED_GENERIC, QW_SCHED_FUSED, QW_SCHED_BLOCKED, QW_SCHED_RESIDENT, QW_SCHED_TILED = 0, 1, 2, 3, 4, 5
 QW_INFO_LAUNCHES, QW_INFO_TIME, QW_INFO_LAST_SCHEDULE, QW_INFO_LAST_K, QW_INFO_STATE_BYTES, QW_INFO_WINDOW, \
     QW_INFO_SITES_TOUCHED = range(7)
-QW_OPT_MAX_CTAS, QW_OPT_BLOCKED1D_KERNEL = 0, 1
+QW_OPT_MAX_CTAS, QW_OPT_BLOCKED1D_KERNEL, QW_OPT_TILED2D_KERNEL = 0, 1, 2
 
 # every symbol include/qw.h declares (tests/test_abi.py checks the header against this list)
 SYMBOLS = (

@@ -468,19 +468,21 @@ int qw_step(qw_sim *s, int64_t n) {
     if (sched == QW_SCHED_TILED && !tiled2d_eligible(s))
         return fail(QW_EUNSUPPORTED, "the tiled schedule needs a uniform coin without phases or link mask on a 2D lattice of "
                                      ">= 32 x 32 sites (diagonal lattice: a torus, or an open lattice with a delta start)");
-    if (sched == QW_SCHED_TILED && s->sched_k != 0 && s->sched_k != 2 && s->sched_k != 4 && s->sched_k != 6 && s->sched_k != 8)
-        return fail(QW_EINVAL, "the tiled schedule takes k = 2, 4, 6 or 8 (got %d)", s->sched_k);
+    const bool stream2d = sched == QW_SCHED_TILED && s->tiled2d_kernel != 1 && stream2d_eligible(s);
+    if (sched == QW_SCHED_TILED && (s->sched_k < 0 || s->sched_k % 2 != 0 || s->sched_k > (stream2d ? stream2d_max_k(s) : 8)))
+        return fail(QW_EINVAL, "the tiled schedule takes an even k <= %d here (got %d)", stream2d ? stream2d_max_k(s) : 8, s->sched_k);
     int64_t remaining = n;
     s->last_sched = sched; s->last_k = 1;
     if (sched == QW_SCHED_TILED) {
         // k-step launches, then the even part of the remainder; an odd last step goes through the fused kernel below
-        const int kmax = s->sched_k > 0 ? s->sched_k : (s->dtype == QW_C128 ? 6 : 8);   // measured optima on B200 (profiles/)
+        // measured optima on B200 (profiles/): streaming kernel 8 / 8, CTA tiles 8 (complex64) / 6 (complex128)
+        const int kmax = s->sched_k > 0 ? s->sched_k : (stream2d ? 8 : (s->dtype == QW_C128 ? 6 : 8));
         s->last_k = kmax;
         while (remaining >= 2) {
             const int kk = (int)(remaining >= kmax ? kmax : remaining / 2 * 2);
             if (!tiled2d_diag_open_ok(s, kk)) break;       // the cone reaches a wall: the fused kernel (which has wall code) takes over
             const Box box = step_box(s, kk);
-            int rc = launch_step_tiled2d(s, s->cur, 1 - s->cur, kk, box);
+            int rc = stream2d ? launch_step_stream2d(s, s->cur, 1 - s->cur, kk, box) : launch_step_tiled2d(s, s->cur, 1 - s->cur, kk, box);
             if (rc) return rc;
             s->cur ^= 1; s->t += kk; s->radius += kk; remaining -= kk;
         }
@@ -626,6 +628,10 @@ int qw_set_option(qw_sim *s, int key, int64_t value) {
         case QW_OPT_BLOCKED1D_KERNEL:
             if (value < 0 || value > 2) return fail(QW_EINVAL, "QW_OPT_BLOCKED1D_KERNEL must be 0 (auto), 1 (halo tiles) or 2 (chained tiles)");
             s->blocked1d_kernel = (int)value;
+            break;
+        case QW_OPT_TILED2D_KERNEL:
+            if (value < 0 || value > 2) return fail(QW_EINVAL, "QW_OPT_TILED2D_KERNEL must be 0 (auto), 1 (CTA tiles) or 2 (streaming warps)");
+            s->tiled2d_kernel = (int)value;
             break;
         default: return fail(QW_EINVAL, "unknown option key %d", key);
     }

@@ -84,6 +84,7 @@ struct qw_sim {
     // schedule
     int max_ctas;            // QW_OPT_MAX_CTAS: cap on the grid of the persistent kernels (0 = all SMs)
     int blocked1d_kernel;    // QW_OPT_BLOCKED1D_KERNEL: 0 = cheaper of the two, 1 = halo tiles, 2 = chained tiles (rings)
+    int tiled2d_kernel;      // QW_OPT_TILED2D_KERNEL: 0 = streaming kernel where it applies, 1 = register tiles, 2 = streaming
     int sched, sched_k;
     int last_sched, last_k;
     long long launches;
@@ -181,6 +182,14 @@ bool tiled2d_diag_open_ok(const qw_sim *s, int k);   // open diagonal lattice: k
 int launch_step_tiled2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 int launch_tiled2d_f32(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 int launch_tiled2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
+
+// qw_step_stream2d_*.cu : k in {2,..,12} (even) steps per launch, every warp streams down a strip of columns with a
+// K-level pipeline of rows in REGISTERS (uniform coin, 2D natural lattice); the 2D AUTO schedule where it applies.
+bool stream2d_eligible(const qw_sim *s);
+int stream2d_max_k(const qw_sim *s);
+int launch_step_stream2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
+int launch_stream2d_f32(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
+int launch_stream2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 
 // qw_reduce.cu
 int launch_probabilities(qw_sim *s, const void *state, void *out_dev);

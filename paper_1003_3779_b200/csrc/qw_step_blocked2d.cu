@@ -319,6 +319,18 @@ int launch_step_tiled2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &bo
     return s->dtype == QW_C128 ? launch_tiled2d_f64(s, in_buf, out_buf, k, box) : launch_tiled2d_f32(s, in_buf, out_buf, k, box);
 }
 
+// Streaming schedule (qw_step_stream2d.cuh): natural lattice, uniform coin; same ghost ring as the tiles.
+bool stream2d_eligible(const qw_sim *s) { return blocked2d_eligible(s); }
+int stream2d_max_k(const qw_sim *s) { return s->dtype == QW_C128 ? 8 : 12; }
+
+int launch_step_stream2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
+    if (s->g.boundary == QW_PERIODIC) {
+        int rc = launch_ghost_refresh(s, in_buf);
+        if (rc) return rc;
+    }
+    return s->dtype == QW_C128 ? launch_stream2d_f64(s, in_buf, out_buf, k, box) : launch_stream2d_f32(s, in_buf, out_buf, k, box);
+}
+
 int launch_step_blocked2d(qw_sim *s, int in_buf, int out_buf, int k) {
     const Geom &g = s->g;
     if (k < 1 || k > blocked2d_max_k(s)) return fail(QW_EINVAL, "blocked 2D step depth %d outside [1, %d]", k, blocked2d_max_k(s));

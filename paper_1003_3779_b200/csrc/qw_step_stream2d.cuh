@@ -1,0 +1,358 @@
+// qw_step_stream2d.cuh — streaming temporally blocked 2D step: K applications of U = S (C (x) I)
+// (eq. 7 with the shift of PAPER.md:88 eq. 8) per HBM round trip, uniform coin, natural lattice.
+// Included by one translation unit per dtype.
+//
+// Every WARP works alone (no barrier, no shared-memory exchange between warps).  A warp owns a STRIP of HN = 32*RN
+// columns (lane l: columns l*RN .. l*RN+RN-1) and streams DOWN the rows of a segment of that strip.  In its registers
+// it keeps, for every time level 1 .. K, the one row of that level that is still incomplete: a pipeline of K coin
+// applications through which every row passes once.  With row r of level 0 (the input) arriving,
+//     level l (l = 0 .. K-1) applies the coin (eq. 1) to its row r - l, which the level below has just completed, and
+//     hands the four components on to level l + 1 (eq. 8):   phi_1 -> row r-l+1   (parked until that row completes)
+//                                                             phi_0 -> row r-l, one column to the right (lane shuffle)
+//                                                             phi_3 -> row r-l, one column to the left  (lane shuffle)
+//                                                             phi_2 -> row r-l-1: its last missing component
+//     so row r-l-1 of level l+1 is complete and level l+1 goes on with it; level K's row r-K is the output row.
+// The shift along m is therefore a matter of WHEN a register is consumed (no data moves, no halo along m, no
+// synchronisation); only the shift along n crosses lanes: 2 complex shuffles per level and row.  The unknown outside
+// of a strip travels one column per level, so the K outermost columns on each side are a halo (valid = HN - 2K).
+// A segment of rows [a, b) is fed rows a-K .. b+K-1 (the pipeline fills and drains over 2K rows).
+//
+// Memory: each lane copies its own 16-byte pieces of the next input rows into a per-warp ring in shared memory with
+// cp.async (several rows ahead) and reads them back itself, so there is no cross-lane dependency; output rows go from
+// registers to global memory as 16-byte stores.  Halos (rows and columns) come from the ghost ring of the state
+// buffers (periodic: refreshed before each launch).
+//
+// Walls (open lattice = broken outward links, PAPER.md:94-101 with RBL = 0): the outgoing component stays on its site
+// with the opposite coin (3 - c).  Only the units that can see a wall run the instance with the wall code.
+#pragma once
+
+#include <type_traits>
+
+#include "qw_coin.cuh"
+
+namespace qw {
+
+// Launch shape per dtype and block depth K: RN = columns per lane (strip of 32*RN columns; a lane's row segment is a
+// whole number of 16-byte vectors), WPC = warps per CTA (one CTA per SM; 12 warps leave 168 registers per thread, 8 leave
+// 255 — the pipeline holds 4*RN complex amplitudes per level), RING / PF = rows of the per-warp input ring in shared
+// memory / prefetch distance (WPC * RING * 4 * 32*RN * sizeof(complex) <= 192 KiB).
+template <typename R, int K> struct S2dShape;
+template <int K> struct S2dShape<float, K> {
+    static constexpr int RN = 2, WPC = (K <= 4) ? 12 : 8, RING = 8, PF = 6;
+};
+template <int K> struct S2dShape<double, K> {
+    static constexpr int RN = (K <= 4) ? 2 : 1, WPC = (K <= 2) ? 12 : 8, RING = (K <= 4) ? 4 : 8, PF = RING - 1;
+};
+
+template <typename R>
+struct Stream2dArgs {
+    const typename Cx<R>::T *in;  // site (0,0) of walk 0, plane 0 of the input buffer
+    typename Cx<R>::T *out;       // ... of the output buffer
+    long long em, en, pitch, walk_stride, plane_stride;
+    long long max_col;            // largest column index a lane may address (row allocation end), a multiple of RN
+    int batch;
+    int strip0, strips;           // launched range of the global strip grid: strip j owns columns [j*V, (j+1)*V)
+    long long row_lo, row_hi;     // launched rows (inclusive), cut into `segs` segments of `seg_len` rows
+    long long seg_len;
+    int segs;
+    long long units;              // batch * segs * strips
+    R coin[32];
+    R coin_last[32];              // deferred scale of the named coins: coin * scale^(K-1) (qw_coin.cuh: apply_coin_bare)
+    R ratio;                      // Grover-like: (d - g) / g
+    long long dia_m, dia_n, dia_r;   // light-cone diamond (dia_r < 0: none), as in qw_step_tiled2d.cuh
+};
+
+namespace s2d {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(void *dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async16_s(uint32_t dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <typename R> __device__ __forceinline__ cplx<R> shfl_up1(cplx<R> v) {
+    v.re = __shfl_up_sync(0xffffffffu, v.re, 1);
+    v.im = __shfl_up_sync(0xffffffffu, v.im, 1);
+    return v;
+}
+template <typename R> __device__ __forceinline__ cplx<R> shfl_down1(cplx<R> v) {
+    v.re = __shfl_down_sync(0xffffffffu, v.re, 1);
+    v.im = __shfl_down_sync(0xffffffffu, v.im, 1);
+    return v;
+}
+
+// A lane's row segment of RN consecutive sites <-> 16-byte vectors
+template <int RN> __device__ __forceinline__ void load_seg(const float2 *src, cplx<float> (&dst)[RN]) {
+    static_assert(RN % 2 == 0, "complex64 segments are moved as float4");
+#pragma unroll
+    for (int q = 0; q < RN / 2; ++q) {
+        const float4 v = *reinterpret_cast<const float4 *>(src + 2 * q);
+        dst[2 * q] = cplx<float>{v.x, v.y};
+        dst[2 * q + 1] = cplx<float>{v.z, v.w};
+    }
+}
+template <int RN> __device__ __forceinline__ void load_seg(const double2 *src, cplx<double> (&dst)[RN]) {
+#pragma unroll
+    for (int j = 0; j < RN; ++j) { const double2 v = src[j]; dst[j] = cplx<double>{v.x, v.y}; }
+}
+template <int RN> __device__ __forceinline__ void store_seg(float2 *dst, const cplx<float> (&src)[RN]) {
+#pragma unroll
+    for (int q = 0; q < RN / 2; ++q)
+        *reinterpret_cast<float4 *>(dst + 2 * q) = make_float4(src[2 * q].re, src[2 * q].im, src[2 * q + 1].re, src[2 * q + 1].im);
+}
+template <int RN> __device__ __forceinline__ void store_seg(double2 *dst, const cplx<double> (&src)[RN]) {
+#pragma unroll
+    for (int j = 0; j < RN; ++j) dst[j] = make_double2(src[j].re, src[j].im);
+}
+
+// What level l+1 holds of its incomplete rows between two cascades (q = the row level l coins next):
+//   c0, c3   of row q-1 (already shifted along n)     c1[p]   of row q-1     c1[p^1]   of row q     (p = parity of the cascade)
+template <typename R, int RN> struct Level { cplx<R> c0[RN], c3[RN], c1[2][RN]; };
+
+// The coin in two stages, so that a level's parked registers can be REUSED IN PLACE: the front stage reads the four
+// components of a site and leaves four intermediates, the back stage turns them into phi_0 .. phi_3.  For the radix-2
+// coins (H (x) H, DFT) these are the two butterfly levels of qw_coin.cuh — the same operations in the same order, so the
+// results are bit for bit those of apply_coin_bare / apply_coin; the other coins are evaluated completely by the front stage.
+template <typename R, int KIND, bool LAST>
+__device__ __forceinline__ void coin_front(const R *C, const R *Clast, R ratio, const cplx<R> (&v)[4], cplx<R> (&t)[4]) {
+    if constexpr (KIND == COIN_HXH4 && !LAST) {
+        t[0] = cx_add(v[0], v[1]); t[1] = cx_sub(v[0], v[1]); t[2] = cx_add(v[2], v[3]); t[3] = cx_sub(v[2], v[3]);
+    } else if constexpr (KIND == COIN_HXH4 && LAST) {
+        const R h = Clast[0];
+        const cplx<R> s1 = cx_scale(h, v[1]), s3 = cx_scale(h, v[3]);
+        t[0] = cx_fma_r(h, v[0], s1); t[1] = cx_fms_r(h, v[0], s1); t[2] = cx_fma_r(h, v[2], s3); t[3] = cx_fms_r(h, v[2], s3);
+    } else if constexpr (KIND == COIN_DFT4 && !LAST) {
+        t[0] = cx_add(v[0], v[2]); t[1] = cx_sub(v[0], v[2]); t[2] = cx_add(v[1], v[3]); t[3] = cx_muli(cx_sub(v[1], v[3]));
+    } else if constexpr (KIND == COIN_DFT4 && LAST) {
+        const R h = Clast[0];
+        const cplx<R> s2 = cx_scale(h, v[2]), s3 = cx_scale(h, v[3]);
+        t[0] = cx_fma_r(h, v[0], s2); t[1] = cx_fms_r(h, v[0], s2); t[2] = cx_fma_r(h, v[1], s3); t[3] = cx_muli(cx_fms_r(h, v[1], s3));
+    } else {
+#pragma unroll
+        for (int a = 0; a < 4; ++a) t[a] = v[a];
+        if constexpr (KIND == COIN_GENERAL) apply_coin<R, 4, KIND>(C, t);
+        else if constexpr (LAST) apply_coin<R, 4, KIND>(Clast, t);
+        else apply_coin_bare<R, KIND>(ratio, t);
+    }
+}
+template <typename R, int KIND, int A>
+__device__ __forceinline__ cplx<R> coin_back(const cplx<R> (&t)[4]) {
+    if constexpr (KIND == COIN_HXH4 || KIND == COIN_DFT4)
+        return A == 0 ? cx_add(t[0], t[2]) : A == 1 ? cx_add(t[1], t[3]) : A == 2 ? cx_sub(t[0], t[2]) : cx_sub(t[1], t[3]);
+    else
+        return t[A];
+}
+
+// One cascade: input row r (complete, in x) passes level 0, the row it completes passes level 1, ...; emit(out) is called
+// with row r-K of level K.  PAR = parity of the cascade count (which of the two phi_1 slots is due).
+// Order inside a level boundary (what keeps the register allocation free of moves): phi_2 of level l first; with it the
+// completed row of level l+1 goes through ITS front stage, which is the last reader of the parked registers; only then
+// the back stage of level l produces phi_0, phi_1, phi_3 — straight into those registers.
+// WALL: r = the input row as a row of the lattice (rows 0 / em-1 are walls), jl / jr = this lane's local column of
+// lattice column 0 / en-1 (or -1).
+template <typename R, int KIND, int K, int RN, bool WALL, int PAR, typename Emit>
+__device__ __forceinline__ void cascade(const cplx<R> (&x)[4][RN], Level<R, RN> (&S)[K], const R *C, const R *Clast, R ratio,
+                                        long long r, long long em, int jl, int jr, Emit emit) {
+    cplx<R> t[RN][4];
+#pragma unroll
+    for (int j = 0; j < RN; ++j) {
+        const cplx<R> v[4] = {x[0][j], x[1][j], x[2][j], x[3][j]};
+        coin_front<R, KIND, K == 1>(C, Clast, ratio, v, t[j]);
+    }
+#pragma unroll
+    for (int l = 0; l < K; ++l) {
+        const long long q = r - l;                     // the lattice row level l is coining
+        // ---- phi_2 of row q completes row q-1 of level l+1
+        cplx<R> c2n[RN];
+#pragma unroll
+        for (int j = 0; j < RN; ++j) c2n[j] = coin_back<R, KIND, 2>(t[j]);
+        cplx<R> y2w[RN];
+        if constexpr (WALL) {
+#pragma unroll
+            for (int j = 0; j < RN; ++j) y2w[j] = c2n[j];
+            if (q == em) {                             // bottom wall: phi_1 of row em-1 (parked for row em) -> c2 of row em-1
+#pragma unroll
+                for (int j = 0; j < RN; ++j) c2n[j] = S[l].c1[PAR ^ 1][j];
+            }
+        }
+        cplx<R> tn[RN][4];
+        if (l + 1 < K) {
+#pragma unroll
+            for (int j = 0; j < RN; ++j) {
+                const cplx<R> v[4] = {S[l].c0[j], S[l].c1[PAR][j], c2n[j], S[l].c3[j]};
+                if (l + 2 == K) coin_front<R, KIND, true>(C, Clast, ratio, v, tn[j]);
+                else coin_front<R, KIND, false>(C, Clast, ratio, v, tn[j]);
+            }
+        } else {
+            cplx<R> out[4][RN];
+#pragma unroll
+            for (int j = 0; j < RN; ++j) { out[0][j] = S[l].c0[j]; out[1][j] = S[l].c1[PAR][j]; out[2][j] = c2n[j]; out[3][j] = S[l].c3[j]; }
+            emit(out);
+        }
+        // ---- phi_0, phi_1, phi_3 of row q, shifted (eq. 8), into the registers that have just been read for the last time
+        cplx<R> y0[RN], y3[RN];
+#pragma unroll
+        for (int j = 0; j < RN; ++j) { y0[j] = coin_back<R, KIND, 0>(t[j]); y3[j] = coin_back<R, KIND, 3>(t[j]); }
+#pragma unroll
+        for (int j = 0; j < RN; ++j) S[l].c1[PAR][j] = coin_back<R, KIND, 1>(t[j]);
+        S[l].c0[0] = shfl_up1(y0[RN - 1]);             // phi_0 of the lane to the left enters column 0
+        S[l].c3[RN - 1] = shfl_down1(y3[0]);           // phi_3 of the lane to the right enters column RN-1
+#pragma unroll
+        for (int j = 1; j < RN; ++j) { S[l].c0[j] = y0[j - 1]; S[l].c3[j - 1] = y3[j]; }
+        if constexpr (WALL) {
+            // reflecting walls (RBL = 0): the outgoing component stays with the opposite coin
+#pragma unroll
+            for (int j = 0; j < RN; ++j) {
+                if (jl == j) S[l].c0[j] = y3[j];       // left wall:  phi_3 -> c0 of the same site
+                if (jr == j) S[l].c3[j] = y0[j];       // right wall: phi_0 -> c3 of the same site
+            }
+            if (q == 0) {                              // top wall: phi_2 -> c1 of row 0 (instead of phi_1 of row -1)
+#pragma unroll
+                for (int j = 0; j < RN; ++j) S[l].c1[PAR ^ 1][j] = y2w[j];
+            }
+        }
+        if (l + 1 < K) {
+#pragma unroll
+            for (int j = 0; j < RN; ++j) {
+#pragma unroll
+                for (int a = 0; a < 4; ++a) t[j][a] = tn[j][a];
+            }
+        }
+    }
+}
+
+}  // namespace s2d
+
+template <typename R, int K> constexpr size_t stream2d_smem_bytes() {
+    return (size_t)S2dShape<R, K>::WPC * S2dShape<R, K>::RING * 4 * (32 * S2dShape<R, K>::RN) * sizeof(typename Cx<R>::T);
+}
+
+template <typename R, int KIND, bool OPEN, int K>
+__global__ void __launch_bounds__(S2dShape<R, K>::WPC * 32, 1)
+step_stream2d_kernel(const Stream2dArgs<R> a) {
+    typedef typename Cx<R>::T V;
+    constexpr int RN = S2dShape<R, K>::RN, HN = 32 * RN, VN = HN - 2 * K;
+    constexpr int WPC = S2dShape<R, K>::WPC, RING = S2dShape<R, K>::RING, PF = S2dShape<R, K>::PF;
+    static_assert(VN > 0, "block depth too large for the strip");
+    static_assert(sizeof(V) == 16 || K % 2 == 0, "complex64 strips need an even halo (16-byte aligned lane segments)");
+    static_assert(K % RN == 0, "the halo must be a whole number of lane segments");
+    static_assert((RING & (RING - 1)) == 0 && PF < RING, "ring depth");
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    V *ring = reinterpret_cast<V *>(smem_raw) + (size_t)wid * (RING * 4 * HN) + lane * RN;   // ring[slot][plane][HN], this lane's segment
+    const uint32_t ring_s = s2d::smem_u32(ring);
+    const long long nwarps = (long long)gridDim.x * WPC;
+    const long long per_walk = (long long)a.segs * a.strips;
+    const R *C = a.coin;
+
+    auto run = [&](auto wall_tag, long long w, long long a0, long long b0, long long n0) {
+        constexpr bool WALL = decltype(wall_tag)::value;
+        constexpr uint32_t PLB = HN * sizeof(V), SLOTB = 4 * PLB;             // bytes of a plane row / of a ring slot
+        const long long col = n0 + lane * RN;
+        const long long lcol = col <= a.max_col ? col : a.max_col;             // lanes beyond the row allocation re-read its end
+        // running byte pointers (plane 0): the next input row to fetch, the next output row to store
+        const char *gp = reinterpret_cast<const char *>(a.in + w * a.walk_stride + (a0 - K) * a.pitch + lcol);
+        char *op = reinterpret_cast<char *>(a.out + w * a.walk_stride + a0 * a.pitch + col);
+        const long long planeb = a.plane_stride * (long long)sizeof(V);
+        const long long rowb = a.pitch * (long long)sizeof(V);
+        const long long jl_ = -col, jr_ = a.en - 1 - col;
+        const int jl = (jl_ >= 0 && jl_ < RN) ? (int)jl_ : -1, jr = (jr_ >= 0 && jr_ < RN) ? (int)jr_ : -1;
+        const bool st_lane = (lane * RN >= K) && (lane * RN + RN <= HN - K) && col < a.en;
+        const bool st_full = col + RN <= a.en;
+        const int nrows = (int)(b0 - a0) + 2 * K;
+        uint32_t fslot = 0, lslot = 0;                                         // ring slot offsets (bytes) of the next fetch / next read
+
+        s2d::Level<R, RN> S[K];
+#pragma unroll
+        for (int l = 0; l < K; ++l) {
+#pragma unroll
+            for (int j = 0; j < RN; ++j)
+                S[l].c0[j] = S[l].c3[j] = S[l].c1[0][j] = S[l].c1[1][j] = cplx<R>{0, 0};
+        }
+        auto fetch = [&](bool live) {              // the next input row -> the next ring slot
+            if (live) {
+                const char *g = gp;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+#pragma unroll
+                    for (int q = 0; q < (int)(RN * sizeof(V) / 16); ++q)
+                        s2d::cp_async16_s(ring_s + fslot + c * PLB + 16 * q, g + 16 * q);
+                    g += planeb;
+                }
+                gp += rowb;
+            }
+            fslot = (fslot + SLOTB) & (RING * SLOTB - 1);
+            s2d::cp_async_commit();
+        };
+        auto one = [&](auto par_tag, int i) {
+            constexpr int PAR = decltype(par_tag)::value;
+            fetch(i + PF < nrows);
+            s2d::cp_async_wait<PF>();
+            cplx<R> x[4][RN];
+            const V *sl = reinterpret_cast<const V *>(reinterpret_cast<const char *>(ring) + lslot);
+            lslot = (lslot + SLOTB) & (RING * SLOTB - 1);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) s2d::load_seg<RN>(sl + c * HN, x[c]);
+            s2d::cascade<R, KIND, K, RN, WALL, PAR>(x, S, C, a.coin_last, a.ratio, a0 - K + i, a.em, jl, jr,
+                                                    [&](const cplx<R> (&o)[4][RN]) {
+                if (i >= 2 * K && i < nrows) {     // output row a0 + (i - 2K)
+                    if (st_lane) {
+                        char *o_ = op;
+                        if (st_full) {
+#pragma unroll
+                            for (int c = 0; c < 4; ++c) { s2d::store_seg<RN>(reinterpret_cast<V *>(o_), o[c]); o_ += planeb; }
+                        } else {
+#pragma unroll
+                            for (int c = 0; c < 4; ++c) {
+#pragma unroll
+                                for (int j = 0; j < RN; ++j)
+                                    if (col + j < a.en) cx_store<R>(reinterpret_cast<V *>(o_) + j, o[c][j]);
+                                o_ += planeb;
+                            }
+                        }
+                    }
+                    op += rowb;
+                }
+            });
+        };
+#pragma unroll 1
+        for (int i = 0; i < PF; ++i) fetch(i < nrows);
+#pragma unroll 1
+        for (int i = 0; i < nrows; i += 2) {       // always two cascades per trip (fixed register roles); a surplus odd row is not stored
+            one(std::integral_constant<int, 0>{}, i);
+            one(std::integral_constant<int, 1>{}, i + 1);
+        }
+        s2d::cp_async_wait<0>();
+    };
+
+    for (long long u = (long long)blockIdx.x * WPC + wid; u < a.units; u += nwarps) {
+        const long long w = u / per_walk;
+        const long long rr = u - w * per_walk;
+        const int seg = (int)(rr / a.strips);
+        const int strip = a.strip0 + (int)(rr - (long long)seg * a.strips);
+        const long long a0 = a.row_lo + seg * a.seg_len;
+        long long b0 = a0 + a.seg_len;
+        if (b0 > a.row_hi + 1) b0 = a.row_hi + 1;
+        if (a0 >= b0) continue;
+        const long long n_lo = (long long)strip * VN, n0 = n_lo - K;
+        if (a.dia_r >= 0) {                        // light-cone diamond: units whose outputs are all zeros are skipped
+            const long long n_hi = n_lo + VN - 1;
+            const long long dm = a.dia_m < a0 ? a0 - a.dia_m : (a.dia_m > b0 - 1 ? a.dia_m - (b0 - 1) : 0);
+            const long long dn = a.dia_n < n_lo ? n_lo - a.dia_n : (a.dia_n > n_hi ? a.dia_n - n_hi : 0);
+            if (dm + dn > a.dia_r) continue;
+        }
+        if constexpr (OPEN) {                      // only the units that can see a wall pay for the wall code
+            if ((a0 - K <= 0) || (b0 + K >= a.em) || (n0 <= 0) || (n0 + HN >= a.en)) run(std::true_type{}, w, a0, b0, n0);
+            else run(std::false_type{}, w, a0, b0, n0);
+        } else {
+            run(std::false_type{}, w, a0, b0, n0);
+        }
+    }
+}
+
+}  // namespace qw
