@@ -112,6 +112,7 @@ template <int RN> __device__ __forceinline__ void store_seg(double2 *dst, const 
 // What level l+1 holds of its incomplete rows between two cascades (q = the row level l coins next):
 //   c0, c3   of row q-1 (already shifted along n)     c1[p]   of row q-1     c1[p^1]   of row q     (p = parity of the cascade)
 template <typename R, int RN> struct Level { cplx<R> c0[RN], c3[RN], c1[2][RN]; };
+template <typename R, int RN> struct Row { cplx<R> c[4][RN]; };      // the four components of a lane's row segment
 
 // The coin in two stages, so that a level's parked registers can be REUSED IN PLACE: the front stage reads the four
 // components of a site and leaves four intermediates, the back stage turns them into phi_0 .. phi_3.  For the radix-2
@@ -250,8 +251,11 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
     const long long per_walk = (long long)a.segs * a.strips;
     const R *C = a.coin;
 
-    auto run = [&](auto wall_tag, long long w, long long a0, long long b0, long long n0) {
-        constexpr bool WALL = decltype(wall_tag)::value;
+    // EDGE = the unit can see a wall (open lattice) or the right end of the rows (a lane segment may be cut by column
+    // en): only that instance carries the wall code and the element-wise stores.
+    auto run = [&](auto edge_tag, long long w, long long a0, long long b0, long long n0) {
+        constexpr bool EDGE = decltype(edge_tag)::value;
+        constexpr bool WALL = EDGE && OPEN;
         constexpr uint32_t PLB = HN * sizeof(V), SLOTB = 4 * PLB;             // bytes of a plane row / of a ring slot
         const long long col = n0 + lane * RN;
         const long long lcol = col <= a.max_col ? col : a.max_col;             // lanes beyond the row allocation re-read its end
@@ -263,9 +267,10 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
         const long long jl_ = -col, jr_ = a.en - 1 - col;
         const int jl = (jl_ >= 0 && jl_ < RN) ? (int)jl_ : -1, jr = (jr_ >= 0 && jr_ < RN) ? (int)jr_ : -1;
         const bool st_lane = (lane * RN >= K) && (lane * RN + RN <= HN - K) && col < a.en;
-        const bool st_full = col + RN <= a.en;
+        const bool st_full = col + RN <= a.en;                                 // always true in a unit that is not EDGE
         const int nrows = (int)(b0 - a0) + 2 * K;
         uint32_t fslot = 0, lslot = 0;                                         // ring slot offsets (bytes) of the next fetch / next read
+        int fleft = nrows;                                                     // input rows not yet fetched
 
         s2d::Level<R, RN> S[K];
 #pragma unroll
@@ -274,8 +279,8 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
             for (int j = 0; j < RN; ++j)
                 S[l].c0[j] = S[l].c3[j] = S[l].c1[0][j] = S[l].c1[1][j] = cplx<R>{0, 0};
         }
-        auto fetch = [&](bool live) {              // the next input row -> the next ring slot
-            if (live) {
+        auto fetch = [&]() {                       // the next input row -> the next ring slot
+            if (fleft > 0) {
                 const char *g = gp;
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -286,46 +291,54 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
                 }
                 gp += rowb;
             }
+            --fleft;
             fslot = (fslot + SLOTB) & (RING * SLOTB - 1);
             s2d::cp_async_commit();
         };
-        auto one = [&](auto par_tag, int i) {
-            constexpr int PAR = decltype(par_tag)::value;
-            fetch(i + PF < nrows);
-            s2d::cp_async_wait<PF>();
-            cplx<R> x[4][RN];
+        auto take = [&](s2d::Row<R, RN> &x) {      // the next ring slot -> registers (the lane reads what it copied itself)
             const V *sl = reinterpret_cast<const V *>(reinterpret_cast<const char *>(ring) + lslot);
             lslot = (lslot + SLOTB) & (RING * SLOTB - 1);
 #pragma unroll
-            for (int c = 0; c < 4; ++c) s2d::load_seg<RN>(sl + c * HN, x[c]);
-            s2d::cascade<R, KIND, K, RN, WALL, PAR>(x, S, C, a.coin_last, a.ratio, a0 - K + i, a.em, jl, jr,
+            for (int c = 0; c < 4; ++c) s2d::load_seg<RN>(sl + c * HN, x.c[c]);
+        };
+        // one cascade on x (input row i of the unit) while the row after it is taken from the ring into xn
+        auto one = [&](auto par_tag, int i, const s2d::Row<R, RN> &x, s2d::Row<R, RN> &xn) {
+            constexpr int PAR = decltype(par_tag)::value;
+            fetch();
+            s2d::cp_async_wait<PF - 1>();
+            take(xn);
+            s2d::cascade<R, KIND, K, RN, WALL, PAR>(x.c, S, C, a.coin_last, a.ratio, a0 - K + i, a.em, jl, jr,
                                                     [&](const cplx<R> (&o)[4][RN]) {
-                if (i >= 2 * K && i < nrows) {     // output row a0 + (i - 2K)
-                    if (st_lane) {
+                const bool row_ok = i >= 2 * K && i < nrows;                   // output row a0 + (i - 2K)
+                if (row_ok && st_lane && (!EDGE || st_full)) {
+                    char *o_ = op;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) { s2d::store_seg<RN>(reinterpret_cast<V *>(o_), o[c]); o_ += planeb; }
+                }
+                if constexpr (EDGE) {
+                    if (row_ok && st_lane && !st_full) {
                         char *o_ = op;
-                        if (st_full) {
 #pragma unroll
-                            for (int c = 0; c < 4; ++c) { s2d::store_seg<RN>(reinterpret_cast<V *>(o_), o[c]); o_ += planeb; }
-                        } else {
+                        for (int c = 0; c < 4; ++c) {
 #pragma unroll
-                            for (int c = 0; c < 4; ++c) {
-#pragma unroll
-                                for (int j = 0; j < RN; ++j)
-                                    if (col + j < a.en) cx_store<R>(reinterpret_cast<V *>(o_) + j, o[c][j]);
-                                o_ += planeb;
-                            }
+                            for (int j = 0; j < RN; ++j)
+                                if (col + j < a.en) cx_store<R>(reinterpret_cast<V *>(o_) + j, o[c][j]);
+                            o_ += planeb;
                         }
                     }
-                    op += rowb;
                 }
+                if (i >= 2 * K) op += rowb;
             });
         };
 #pragma unroll 1
-        for (int i = 0; i < PF; ++i) fetch(i < nrows);
+        for (int i = 0; i < PF; ++i) fetch();
+        s2d::cp_async_wait<PF - 1>();
+        s2d::Row<R, RN> xa, xb;
+        take(xa);
 #pragma unroll 1
         for (int i = 0; i < nrows; i += 2) {       // always two cascades per trip (fixed register roles); a surplus odd row is not stored
-            one(std::integral_constant<int, 0>{}, i);
-            one(std::integral_constant<int, 1>{}, i + 1);
+            one(std::integral_constant<int, 0>{}, i, xa, xb);
+            one(std::integral_constant<int, 1>{}, i + 1, xb, xa);
         }
         s2d::cp_async_wait<0>();
     };
@@ -346,12 +359,10 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
             const long long dn = a.dia_n < n_lo ? n_lo - a.dia_n : (a.dia_n > n_hi ? a.dia_n - n_hi : 0);
             if (dm + dn > a.dia_r) continue;
         }
-        if constexpr (OPEN) {                      // only the units that can see a wall pay for the wall code
-            if ((a0 - K <= 0) || (b0 + K >= a.em) || (n0 <= 0) || (n0 + HN >= a.en)) run(std::true_type{}, w, a0, b0, n0);
-            else run(std::false_type{}, w, a0, b0, n0);
-        } else {
-            run(std::false_type{}, w, a0, b0, n0);
-        }
+        bool edge = n0 + HN >= a.en;               // the strip holds the right end of the rows
+        if constexpr (OPEN) edge = edge || (a0 - K <= 0) || (b0 + K >= a.em) || (n0 <= 0);
+        if (edge) run(std::true_type{}, w, a0, b0, n0);
+        else run(std::false_type{}, w, a0, b0, n0);
     }
 }
 
