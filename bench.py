@@ -122,7 +122,7 @@ def coin_cost(w, sched_name="fused", kdepth=0):
         return instr, flops
     # 2D named coins: scaled evaluation 20 / 16 / 20 instructions; the tiled kernel defers the power-of-two scale:
     # K-1 bare steps (H(x)H, DFT: 16 add; Grover: 6 add + 8 fma) + 1 scaled step per K steps
-    K = kdepth if kdepth in (2, 4, 6, 8) else (8 if w.dtype == np.complex64 else 6)
+    K = kdepth if kdepth in (2, 4, 6, 8, 10, 12) else (8 if w.dtype == np.complex64 else 6)
     def tiled(bare_i, bare_f, full_i, full_f):
         if sched_name == "tiled":
             return ((K - 1) * bare_i + full_i) / K, ((K - 1) * bare_f + full_f) / K
@@ -574,7 +574,7 @@ def run_gpu(args):
     sched_name = {0: "auto", 1: "generic", 2: "fused", 3: "blocked", 4: "resident", 5: "tiled"}.get(sched, str(sched))
     kname = {1: "step_scatter_kernel (generic)", 2: "step_scatter_kernel (fused coin+shift)",
              3: "step_blocked1d_kernel" if w.dim == 1 else "step_blocked2d_kernel", 4: "step_resident1d_kernel",
-             5: "step_tiled2d_kernel"}.get(sched, "?")
+             5: "step_stream2d_kernel" if (w.lattice == qi.NATURAL and "2=1" not in args.opt) else "step_tiled2d_kernel"}.get(sched, "?")
     touched_frac = touched_per_step / site_updates_per_step          # < 1 when the light-cone window skipped work
     if sched in (1, 2):
         touched_gbs = eff_gbs * touched_frac

@@ -180,6 +180,14 @@ int qw_step_inverse(qw_sim *s, int64_t n);
 /* P[w][x] = sum_a |psi[w][x][a]|^2: [batch][site] double (C128) / float (C64). */
 int qw_probabilities(const qw_sim *s, void *out);
 
+/* Ensemble average over the batch: out[x] = (1 / batch) * sum_walks P_walk(x), `sites` reals of the handle's real type
+ * (host or device), sites in row-major order.  This is the averaged distribution of the random-broken-links model
+ * ("random broken links (termed RBL) technique", :221 "without and with broken links"): with
+ * qw_set_random_broken_links every walk of a batch draws its own links, so a batch started from one initial state is
+ * an ensemble of realisations.  Accumulated in double over the walks in order (deterministic).
+ * QW_ESTATE without a state. */
+int qw_probabilities_mean(const qw_sim *s, void *out);
+
 /* Per walk, in double regardless of dtype: 1D {norm, mean, var};
  * 2D {norm, mean_m, mean_n, var_m, var_n, cov_mn}.  Coordinates x_d = index_d - floor(extent_d/2);
  * mean and (population) variance are divided by the computed norm (eq. 4 fixes norm = 1). */

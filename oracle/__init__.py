@@ -12,6 +12,7 @@ from .oracle import (  # noqa: F401
     moments,
     philox4x32_10,
     probabilities,
+    probabilities_mean,
     rbl_mask,
     step,
     step_inverse,

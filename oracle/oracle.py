@@ -42,6 +42,7 @@ def _load():
         lib.qwo_step_inverse.argtypes = lib.qwo_step.argtypes
         lib.qwo_probabilities.argtypes = [ctypes.c_int, i64p, ctypes.c_int64, vp, vp]
         lib.qwo_moments.argtypes = [ctypes.c_int, i64p, ctypes.c_int64, vp, vp]
+        lib.qwo_probabilities_mean.argtypes = [ctypes.c_int, i64p, ctypes.c_int64, vp, vp]
         lib.qwo_dense_unitary.argtypes = [ctypes.c_int, i64p, ctypes.c_int, ctypes.c_int,
                                           ctypes.c_int, vp, vp, vp]
         lib.qwo_step_rbl.argtypes = [ctypes.c_int, i64p, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp,
@@ -51,7 +52,7 @@ def _load():
                                      ctypes.c_double, ctypes.c_uint64, ctypes.c_int64, vp]
         lib.qwo_philox4x32_10.argtypes = [vp, vp, vp]
         lib.qwo_philox4x32_10.restype = None
-        for f in (lib.qwo_step, lib.qwo_step_inverse, lib.qwo_probabilities, lib.qwo_moments,
+        for f in (lib.qwo_step, lib.qwo_step_inverse, lib.qwo_probabilities, lib.qwo_moments, lib.qwo_probabilities_mean,
                   lib.qwo_dense_unitary, lib.qwo_step_rbl, lib.qwo_step_inverse_rbl, lib.qwo_rbl_mask):
             f.restype = ctypes.c_int
         _lib = lib
@@ -115,6 +116,17 @@ def probabilities(extents, state, *, batch=1):
     _state(state, batch, sites, 2 * dim)
     out = np.empty((batch, sites), dtype=np.float64)
     rc = _load().qwo_probabilities(dim, ext, batch, state.ctypes.data, out.ctypes.data)
+    if rc:
+        raise ValueError("oracle rejected the arguments")
+    return out
+
+
+def probabilities_mean(extents, state, *, batch=1):
+    """Pbar[x] = (1/batch) sum_w sum_a |psi[w][x][a]|^2: the ensemble average over the batch."""
+    dim, ext, sites = _ext(extents)
+    _state(state, batch, sites, 2 * dim)
+    out = np.empty((sites,), dtype=np.float64)
+    rc = _load().qwo_probabilities_mean(dim, ext, batch, state.ctypes.data, out.ctypes.data)
     if rc:
         raise ValueError("oracle rejected the arguments")
     return out

@@ -313,6 +313,29 @@ int qwo_probabilities(int dim, const int64_t* extents, int64_t batch, const doub
     return 0;
 }
 
+// Ensemble average over the batch: Pbar[x] = (1/batch) sum_w P[w][x], P as in qwo_probabilities; the
+// averaged distribution of the random-broken-links model, every walk of
+// the batch being one realisation of the links.  Plain definition: sum over the walks in order, then divide.
+int qwo_probabilities_mean(int dim, const int64_t* extents, int64_t batch, const double* state_, double* Pbar) {
+    Lattice L;
+    if (!make_lattice(dim, extents, 0, 0, &L) || batch < 1) return -1;
+    const cplx* state = reinterpret_cast<const cplx*>(state_);
+    const int cd = L.cdim;
+    for (int64_t x = 0; x < L.sites; ++x) {
+        double sum = 0.0;
+        for (int64_t w = 0; w < batch; ++w) {
+            double p = 0.0;
+            for (int a = 0; a < cd; ++a) {
+                const cplx z = state[(w * L.sites + x) * cd + a];
+                p += z.re * z.re + z.im * z.im;
+            }
+            sum += p;
+        }
+        Pbar[x] = sum / (double)batch;
+    }
+    return 0;
+}
+
 // Per walk: 1D {norm, mean, var}; 2D {norm, mean_m, mean_n, var_m, var_n, cov_mn}.
 // Coordinates x_d = index_d - floor(extent_d / 2); moments divided by the computed norm;
 // population variance.  Accumulated in long double so the oracle is the more accurate side.

@@ -475,8 +475,8 @@ int qw_step(qw_sim *s, int64_t n) {
     s->last_sched = sched; s->last_k = 1;
     if (sched == QW_SCHED_TILED) {
         // k-step launches, then the even part of the remainder; an odd last step goes through the fused kernel below
-        // measured optima on B200 (profiles/): streaming kernel 8 / 8, CTA tiles 8 (complex64) / 6 (complex128)
-        const int kmax = s->sched_k > 0 ? s->sched_k : (stream2d ? 8 : (s->dtype == QW_C128 ? 6 : 8));
+        // measured optima on B200 (profiles/), both kernels: 8 (complex64) / 6 (complex128)
+        const int kmax = s->sched_k > 0 ? s->sched_k : (s->dtype == QW_C128 ? 6 : 8);
         s->last_k = kmax;
         while (remaining >= 2) {
             const int kk = (int)(remaining >= kmax ? kmax : remaining / 2 * 2);
@@ -584,6 +584,24 @@ int qw_probabilities(const qw_sim *cs, void *out) {
     int rc = ensure_scratch(s, bytes);
     if (rc) return rc;
     rc = launch_probabilities(s, state_ptr(s, s->cur), s->scratch);
+    if (rc) return rc;
+    QW_CUDA(cudaMemcpyAsync(out, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
+    QW_CUDA(cudaStreamSynchronize(s->stream));
+    return QW_OK;
+}
+
+int qw_probabilities_mean(const qw_sim *cs, void *out) {
+    clear_error();
+    qw_sim *s = const_cast<qw_sim *>(cs);
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
+    if (!out) return fail(QW_EINVAL, "out is NULL");
+    if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
+    const size_t bytes = (size_t)s->g.sites * (s->esize / 2);
+    if (is_device_ptr(out)) return launch_probabilities_mean(s, state_ptr(s, s->cur), out);
+    int rc = ensure_scratch(s, bytes);
+    if (rc) return rc;
+    rc = launch_probabilities_mean(s, state_ptr(s, s->cur), s->scratch);
     if (rc) return rc;
     QW_CUDA(cudaMemcpyAsync(out, s->scratch, bytes, cudaMemcpyDeviceToHost, s->stream));
     QW_CUDA(cudaStreamSynchronize(s->stream));

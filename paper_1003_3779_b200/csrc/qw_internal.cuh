@@ -193,6 +193,7 @@ int launch_stream2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &bo
 
 // qw_reduce.cu
 int launch_probabilities(qw_sim *s, const void *state, void *out_dev);
+int launch_probabilities_mean(qw_sim *s, const void *state, void *out_dev);   // [sites], mean over the batch
 int launch_moments(qw_sim *s, const void *state, double *out_dev);
 
 }  // namespace qw

@@ -96,6 +96,61 @@ static int launch_prob_t(qw_sim *s, const void *state, void *out) {
     return QW_OK;
 }
 
+// Ensemble average over the batch axis: Pbar(x) = (1/B) sum_w P_w(x) (the averaged distribution of the random-broken-links
+// model: every walk of a batch draws its own links).  One thread takes VEC consecutive sites of a lattice
+// row and runs over the walks in order (FP64 accumulation: deterministic, and the mean of complex64 walks loses nothing).
+template <typename R, int CD>
+__global__ void __launch_bounds__(RED_BLOCK)
+prob_mean_kernel(const typename Cx<R>::T *__restrict__ st, R *__restrict__ out, long long batch, long long em, long long en,
+                 long long pitch, long long walk_stride, long long plane_stride, int chunks_per_row) {
+    constexpr int VEC = RedVec<R>::value;
+    const long long blk = blockIdx.x;
+    const long long m = blk / chunks_per_row;
+    const long long n = ((blk - m * chunks_per_row) * RED_BLOCK + threadIdx.x) * VEC;
+    if (n >= en) return;
+    const double inv = 1.0 / (double)batch;
+    R *o = out + m * en + n;
+    if (n + VEC <= en) {
+        double acc[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) acc[v] = 0.0;
+        for (long long w = 0; w < batch; ++w) {
+            double p[VEC];
+            site_probs<R, double, CD, VEC>(st, plane_stride, w * walk_stride + m * pitch + n, p);
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) acc[v] += p[v];
+        }
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) o[v] = (R)(acc[v] * inv);
+    } else {
+        for (int v = 0; n + v < en; ++v) {
+            double acc = 0.0;
+            for (long long w = 0; w < batch; ++w) acc += site_prob1<R, double, CD>(st, plane_stride, w * walk_stride + m * pitch + n + v);
+            o[v] = (R)(acc * inv);
+        }
+    }
+}
+
+template <typename R, int CD>
+static int launch_prob_mean_t(qw_sim *s, const void *state, void *out) {
+    const Geom &g = s->g;
+    constexpr int PER_BLOCK = RED_BLOCK * RedVec<R>::value;
+    const int cpr = (int)((g.en + PER_BLOCK - 1) / PER_BLOCK);
+    const long long blocks = g.em * cpr;
+    if (blocks > 0x7fffffffLL) return fail(QW_EUNSUPPORTED, "lattice too large for one launch");
+    prob_mean_kernel<R, CD><<<(unsigned)blocks, RED_BLOCK, 0, s->stream>>>(
+        static_cast<const typename Cx<R>::T *>(state), static_cast<R *>(out), g.batch, g.em, g.en, g.pitch, g.walk_stride,
+        g.plane_stride, cpr);
+    QW_LAUNCH_CHECK(s, "prob_mean_kernel");
+    return QW_OK;
+}
+
+int launch_probabilities_mean(qw_sim *s, const void *state, void *out) {
+    if (s->dtype == QW_C128)
+        return s->g.cdim == 2 ? launch_prob_mean_t<double, 2>(s, state, out) : launch_prob_mean_t<double, 4>(s, state, out);
+    return s->g.cdim == 2 ? launch_prob_mean_t<float, 2>(s, state, out) : launch_prob_mean_t<float, 4>(s, state, out);
+}
+
 int launch_probabilities(qw_sim *s, const void *state, void *out) {
     if (s->dtype == QW_C128)
         return s->g.cdim == 2 ? launch_prob_t<double, 2>(s, state, out) : launch_prob_t<double, 4>(s, state, out);

@@ -30,6 +30,10 @@
 
 #include "qw_coin.cuh"
 
+#ifndef QW_S2D_WAVE
+#define QW_S2D_WAVE 0
+#endif
+
 namespace qw {
 
 // Launch shape per dtype and block depth K: RN = columns per lane (strip of 32*RN columns; a lane's row segment is a
@@ -37,11 +41,21 @@ namespace qw {
 // 255 — the pipeline holds 4*RN complex amplitudes per level), RING / PF = rows of the per-warp input ring in shared
 // memory / prefetch distance (WPC * RING * 4 * 32*RN * sizeof(complex) <= 192 KiB).
 template <typename R, int K> struct S2dShape;
+// NS = number of levels (the first NS) whose two parked phi_1 rows live in shared memory instead of registers (one 16-byte
+// load and store per level and row): what lets the deep pipelines fit the register file.
+#ifndef QW_S2D_NS10
+#define QW_S2D_NS10 5
+#define QW_S2D_NS12 8
+#endif
 template <int K> struct S2dShape<float, K> {
     static constexpr int RN = 2, WPC = (K <= 4) ? 12 : 8, RING = 8, PF = 6;
+    static constexpr int NS = K <= 8 ? 0 : (K == 10 ? QW_S2D_NS10 : QW_S2D_NS12);
+    static constexpr bool WAVE = QW_S2D_WAVE != 0;
 };
 template <int K> struct S2dShape<double, K> {
     static constexpr int RN = (K <= 4) ? 2 : 1, WPC = (K <= 2) ? 12 : 8, RING = (K <= 4) ? 4 : 8, PF = RING - 1;
+    static constexpr int NS = 0;
+    static constexpr bool WAVE = QW_S2D_WAVE != 0;
 };
 
 template <typename R>
@@ -155,81 +169,139 @@ __device__ __forceinline__ cplx<R> coin_back(const cplx<R> (&t)[4]) {
 // the back stage of level l produces phi_0, phi_1, phi_3 — straight into those registers.
 // WALL: r = the input row as a row of the lattice (rows 0 / em-1 are walls), jl / jr = this lane's local column of
 // lattice column 0 / en-1 (or -1).
-template <typename R, int KIND, int K, int RN, bool WALL, int PAR, typename Emit>
-__device__ __forceinline__ void cascade(const cplx<R> (&x)[4][RN], Level<R, RN> (&S)[K], const R *C, const R *Clast, R ratio,
-                                        long long r, long long em, int jl, int jr, Emit emit) {
-    cplx<R> t[RN][4];
+// ---- one level boundary of a cascade: t = front-stage values of the row (lattice row q) that level L is coining
+// c1s != nullptr: the two parked phi_1 rows of this level live in shared memory, c1s[parity][lane][RN] (this lane's entry).
+template <typename R, int KIND, int K, int RN, bool WALL, int PAR, int L, bool C1S, typename Emit>
+__device__ __forceinline__ void level_step(cplx<R> (&t)[RN][4], Level<R, RN> &S, typename Cx<R>::T *c1s, const R *C, const R *Clast,
+                                           R ratio, long long q, long long em, int jl, int jr, Emit emit) {
+    constexpr int C1P = 32 * RN;                        // elements between the two parities
+    if constexpr (C1S) load_seg<RN>(c1s + PAR * C1P, S.c1[PAR]);
+    // ---- phi_2 of row q completes row q-1 of level L+1
+    cplx<R> c2n[RN];
+#pragma unroll
+    for (int j = 0; j < RN; ++j) c2n[j] = coin_back<R, KIND, 2>(t[j]);
+    cplx<R> y2w[RN];
+    if constexpr (WALL) {
+#pragma unroll
+        for (int j = 0; j < RN; ++j) y2w[j] = c2n[j];
+        if (q == em) {                                 // bottom wall: phi_1 of row em-1 (parked for row em) -> c2 of row em-1
+            if constexpr (C1S) load_seg<RN>(c1s + (PAR ^ 1) * C1P, S.c1[PAR ^ 1]);
+#pragma unroll
+            for (int j = 0; j < RN; ++j) c2n[j] = S.c1[PAR ^ 1][j];
+        }
+    }
+    cplx<R> tn[RN][4];
+    if constexpr (L + 1 < K) {
+#pragma unroll
+        for (int j = 0; j < RN; ++j) {
+            const cplx<R> v[4] = {S.c0[j], S.c1[PAR][j], c2n[j], S.c3[j]};
+            coin_front<R, KIND, L + 2 == K>(C, Clast, ratio, v, tn[j]);
+        }
+    } else {
+        cplx<R> out[4][RN];
+#pragma unroll
+        for (int j = 0; j < RN; ++j) { out[0][j] = S.c0[j]; out[1][j] = S.c1[PAR][j]; out[2][j] = c2n[j]; out[3][j] = S.c3[j]; }
+        emit(out);
+    }
+    // ---- phi_0, phi_1, phi_3 of row q, shifted (eq. 8), into the registers that have just been read for the last time
+    cplx<R> y0[RN], y3[RN];
+#pragma unroll
+    for (int j = 0; j < RN; ++j) { y0[j] = coin_back<R, KIND, 0>(t[j]); y3[j] = coin_back<R, KIND, 3>(t[j]); }
+#pragma unroll
+    for (int j = 0; j < RN; ++j) S.c1[PAR][j] = coin_back<R, KIND, 1>(t[j]);
+    if constexpr (C1S) store_seg<RN>(c1s + PAR * C1P, S.c1[PAR]);
+    S.c0[0] = shfl_up1(y0[RN - 1]);                    // phi_0 of the lane to the left enters column 0
+    S.c3[RN - 1] = shfl_down1(y3[0]);                  // phi_3 of the lane to the right enters column RN-1
+#pragma unroll
+    for (int j = 1; j < RN; ++j) { S.c0[j] = y0[j - 1]; S.c3[j - 1] = y3[j]; }
+    if constexpr (WALL) {
+        // reflecting walls (RBL = 0): the outgoing component stays with the opposite coin
+#pragma unroll
+        for (int j = 0; j < RN; ++j) {
+            if (jl == j) S.c0[j] = y3[j];              // left wall:  phi_3 -> c0 of the same site
+            if (jr == j) S.c3[j] = y0[j];              // right wall: phi_0 -> c3 of the same site
+        }
+        if (q == 0) {                                  // top wall: phi_2 -> c1 of row 0 (instead of phi_1 of row -1)
+#pragma unroll
+            for (int j = 0; j < RN; ++j) S.c1[PAR ^ 1][j] = y2w[j];
+            if constexpr (C1S) store_seg<RN>(c1s + (PAR ^ 1) * C1P, S.c1[PAR ^ 1]);
+        }
+    }
+    if constexpr (L + 1 < K) {
+#pragma unroll
+        for (int j = 0; j < RN; ++j) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a) t[j][a] = tn[j][a];
+        }
+    }
+}
+
+template <typename R, int KIND, int K, int RN>
+__device__ __forceinline__ void front0(const cplx<R> (&x)[4][RN], cplx<R> (&t)[RN][4], const R *C, const R *Clast, R ratio) {
 #pragma unroll
     for (int j = 0; j < RN; ++j) {
         const cplx<R> v[4] = {x[0][j], x[1][j], x[2][j], x[3][j]};
         coin_front<R, KIND, K == 1>(C, Clast, ratio, v, t[j]);
     }
-#pragma unroll
-    for (int l = 0; l < K; ++l) {
-        const long long q = r - l;                     // the lattice row level l is coining
-        // ---- phi_2 of row q completes row q-1 of level l+1
-        cplx<R> c2n[RN];
-#pragma unroll
-        for (int j = 0; j < RN; ++j) c2n[j] = coin_back<R, KIND, 2>(t[j]);
-        cplx<R> y2w[RN];
-        if constexpr (WALL) {
-#pragma unroll
-            for (int j = 0; j < RN; ++j) y2w[j] = c2n[j];
-            if (q == em) {                             // bottom wall: phi_1 of row em-1 (parked for row em) -> c2 of row em-1
-#pragma unroll
-                for (int j = 0; j < RN; ++j) c2n[j] = S[l].c1[PAR ^ 1][j];
-            }
-        }
-        cplx<R> tn[RN][4];
-        if (l + 1 < K) {
-#pragma unroll
-            for (int j = 0; j < RN; ++j) {
-                const cplx<R> v[4] = {S[l].c0[j], S[l].c1[PAR][j], c2n[j], S[l].c3[j]};
-                if (l + 2 == K) coin_front<R, KIND, true>(C, Clast, ratio, v, tn[j]);
-                else coin_front<R, KIND, false>(C, Clast, ratio, v, tn[j]);
-            }
-        } else {
-            cplx<R> out[4][RN];
-#pragma unroll
-            for (int j = 0; j < RN; ++j) { out[0][j] = S[l].c0[j]; out[1][j] = S[l].c1[PAR][j]; out[2][j] = c2n[j]; out[3][j] = S[l].c3[j]; }
-            emit(out);
-        }
-        // ---- phi_0, phi_1, phi_3 of row q, shifted (eq. 8), into the registers that have just been read for the last time
-        cplx<R> y0[RN], y3[RN];
-#pragma unroll
-        for (int j = 0; j < RN; ++j) { y0[j] = coin_back<R, KIND, 0>(t[j]); y3[j] = coin_back<R, KIND, 3>(t[j]); }
-#pragma unroll
-        for (int j = 0; j < RN; ++j) S[l].c1[PAR][j] = coin_back<R, KIND, 1>(t[j]);
-        S[l].c0[0] = shfl_up1(y0[RN - 1]);             // phi_0 of the lane to the left enters column 0
-        S[l].c3[RN - 1] = shfl_down1(y3[0]);           // phi_3 of the lane to the right enters column RN-1
-#pragma unroll
-        for (int j = 1; j < RN; ++j) { S[l].c0[j] = y0[j - 1]; S[l].c3[j - 1] = y3[j]; }
-        if constexpr (WALL) {
-            // reflecting walls (RBL = 0): the outgoing component stays with the opposite coin
-#pragma unroll
-            for (int j = 0; j < RN; ++j) {
-                if (jl == j) S[l].c0[j] = y3[j];       // left wall:  phi_3 -> c0 of the same site
-                if (jr == j) S[l].c3[j] = y0[j];       // right wall: phi_0 -> c3 of the same site
-            }
-            if (q == 0) {                              // top wall: phi_2 -> c1 of row 0 (instead of phi_1 of row -1)
-#pragma unroll
-                for (int j = 0; j < RN; ++j) S[l].c1[PAR ^ 1][j] = y2w[j];
-            }
-        }
-        if (l + 1 < K) {
-#pragma unroll
-            for (int j = 0; j < RN; ++j) {
-#pragma unroll
-                for (int a = 0; a < 4; ++a) t[j][a] = tn[j][a];
-            }
-        }
+}
+
+// level L's slice of the warp's shared-memory phi_1 store (levels 0 .. NS-1): c1s[level][parity][lane][RN]
+template <typename R, int RN, int NS, int L> __device__ __forceinline__ typename Cx<R>::T *c1_of(typename Cx<R>::T *c1s) {
+    return L < NS ? c1s + L * 2 * 32 * RN : nullptr;
+}
+
+template <typename R, int KIND, int K, int RN, int NS, bool WALL, int PAR, int L, typename Emit>
+struct Levels {
+    static __device__ __forceinline__ void run(cplx<R> (&t)[RN][4], Level<R, RN> (&S)[K], typename Cx<R>::T *c1s, const R *C,
+                                               const R *Clast, R ratio, long long r, long long em, int jl, int jr, Emit emit) {
+        level_step<R, KIND, K, RN, WALL, PAR, L, (L < NS)>(t, S[L], c1_of<R, RN, NS, L>(c1s), C, Clast, ratio, r - L, em, jl, jr, emit);
+        if constexpr (L + 1 < K) Levels<R, KIND, K, RN, NS, WALL, PAR, L + 1, Emit>::run(t, S, c1s, C, Clast, ratio, r, em, jl, jr, emit);
     }
+};
+template <typename R, int KIND, int K, int RN, int NS, bool WALL, int PAR, typename Emit>
+__device__ __forceinline__ void cascade(const cplx<R> (&x)[4][RN], Level<R, RN> (&S)[K], typename Cx<R>::T *c1s, const R *C,
+                                        const R *Clast, R ratio, long long r, long long em, int jl, int jr, Emit emit) {
+    cplx<R> t[RN][4];
+    front0<R, KIND, K, RN>(x, t, C, Clast, ratio);
+    Levels<R, KIND, K, RN, NS, WALL, PAR, 0, Emit>::run(t, S, c1s, C, Clast, ratio, r, em, jl, jr, emit);
+}
+
+// Two cascades as a wavefront: row r (parity PAR) runs one level ahead of row r+1 (parity PAR^1), so that at any
+// time two independent dependency chains are in flight in the warp.  Level L of row r+1 reads what level L of row r
+// has parked in the step before: the same order of updates as two cascades one after the other.
+template <typename R, int KIND, int K, int RN, int NS, bool WALL, int PAR, int L, typename EmitA, typename EmitB>
+struct Wave {
+    static __device__ __forceinline__ void run(cplx<R> (&ta)[RN][4], cplx<R> (&tb)[RN][4], Level<R, RN> (&S)[K], typename Cx<R>::T *c1s,
+                                               const R *C, const R *Clast, R ratio, long long r, long long em, int jl, int jr,
+                                               EmitA ea, EmitB eb) {
+        level_step<R, KIND, K, RN, WALL, PAR, L, (L < NS)>(ta, S[L], c1_of<R, RN, NS, L>(c1s), C, Clast, ratio, r - L, em, jl, jr, ea);
+        level_step<R, KIND, K, RN, WALL, PAR ^ 1, L - 1, (L - 1 < NS)>(tb, S[L - 1], c1_of<R, RN, NS, L - 1>(c1s), C, Clast, ratio,
+                                                                      r + 1 - (L - 1), em, jl, jr, eb);
+        if constexpr (L + 1 < K)
+            Wave<R, KIND, K, RN, NS, WALL, PAR, L + 1, EmitA, EmitB>::run(ta, tb, S, c1s, C, Clast, ratio, r, em, jl, jr, ea, eb);
+    }
+};
+// mid() is called as soon as xa has been read for the last time (the caller refills it with the row after next).
+template <typename R, int KIND, int K, int RN, int NS, bool WALL, int PAR, typename Mid, typename EmitA, typename EmitB>
+__device__ __forceinline__ void cascade2(const cplx<R> (&xa)[4][RN], const cplx<R> (&xb)[4][RN], Level<R, RN> (&S)[K],
+                                         typename Cx<R>::T *c1s, const R *C, const R *Clast, R ratio, long long r, long long em,
+                                         int jl, int jr, Mid mid, EmitA ea, EmitB eb) {
+    static_assert(K >= 2, "the wavefront needs two levels");
+    cplx<R> ta[RN][4], tb[RN][4];
+    front0<R, KIND, K, RN>(xa, ta, C, Clast, ratio);
+    mid();
+    level_step<R, KIND, K, RN, WALL, PAR, 0, (0 < NS)>(ta, S[0], c1_of<R, RN, NS, 0>(c1s), C, Clast, ratio, r, em, jl, jr, ea);
+    front0<R, KIND, K, RN>(xb, tb, C, Clast, ratio);
+    Wave<R, KIND, K, RN, NS, WALL, PAR, 1, EmitA, EmitB>::run(ta, tb, S, c1s, C, Clast, ratio, r, em, jl, jr, ea, eb);
+    level_step<R, KIND, K, RN, WALL, PAR ^ 1, K - 1, (K - 1 < NS)>(tb, S[K - 1], c1_of<R, RN, NS, K - 1>(c1s), C, Clast, ratio,
+                                                                  r + 1 - (K - 1), em, jl, jr, eb);
 }
 
 }  // namespace s2d
 
 template <typename R, int K> constexpr size_t stream2d_smem_bytes() {
-    return (size_t)S2dShape<R, K>::WPC * S2dShape<R, K>::RING * 4 * (32 * S2dShape<R, K>::RN) * sizeof(typename Cx<R>::T);
+    return (size_t)S2dShape<R, K>::WPC * (S2dShape<R, K>::RING * 4 + S2dShape<R, K>::NS * 2) * (32 * S2dShape<R, K>::RN) *
+           sizeof(typename Cx<R>::T);
 }
 
 template <typename R, int KIND, bool OPEN, int K>
@@ -237,7 +309,7 @@ __global__ void __launch_bounds__(S2dShape<R, K>::WPC * 32, 1)
 step_stream2d_kernel(const Stream2dArgs<R> a) {
     typedef typename Cx<R>::T V;
     constexpr int RN = S2dShape<R, K>::RN, HN = 32 * RN, VN = HN - 2 * K;
-    constexpr int WPC = S2dShape<R, K>::WPC, RING = S2dShape<R, K>::RING, PF = S2dShape<R, K>::PF;
+    constexpr int WPC = S2dShape<R, K>::WPC, RING = S2dShape<R, K>::RING, PF = S2dShape<R, K>::PF, NS = S2dShape<R, K>::NS;
     static_assert(VN > 0, "block depth too large for the strip");
     static_assert(sizeof(V) == 16 || K % 2 == 0, "complex64 strips need an even halo (16-byte aligned lane segments)");
     static_assert(K % RN == 0, "the halo must be a whole number of lane segments");
@@ -247,6 +319,8 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     V *ring = reinterpret_cast<V *>(smem_raw) + (size_t)wid * (RING * 4 * HN) + lane * RN;   // ring[slot][plane][HN], this lane's segment
     const uint32_t ring_s = s2d::smem_u32(ring);
+    // this lane's entry of the warp's phi_1 store c1s[level][parity][lane][RN] (behind the rings)
+    V *c1s = reinterpret_cast<V *>(smem_raw) + (size_t)WPC * (RING * 4 * HN) + (size_t)wid * (NS * 2 * HN) + lane * RN;
     const long long nwarps = (long long)gridDim.x * WPC;
     const long long per_walk = (long long)a.segs * a.strips;
     const R *C = a.coin;
@@ -279,6 +353,8 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
             for (int j = 0; j < RN; ++j)
                 S[l].c0[j] = S[l].c3[j] = S[l].c1[0][j] = S[l].c1[1][j] = cplx<R>{0, 0};
         }
+#pragma unroll
+        for (int l = 0; l < 2 * NS; ++l) s2d::store_seg<RN>(c1s + l * HN, S[0].c0);
         auto fetch = [&]() {                       // the next input row -> the next ring slot
             if (fleft > 0) {
                 const char *g = gp;
@@ -301,44 +377,61 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
 #pragma unroll
             for (int c = 0; c < 4; ++c) s2d::load_seg<RN>(sl + c * HN, x.c[c]);
         };
-        // one cascade on x (input row i of the unit) while the row after it is taken from the ring into xn
-        auto one = [&](auto par_tag, int i, const s2d::Row<R, RN> &x, s2d::Row<R, RN> &xn) {
-            constexpr int PAR = decltype(par_tag)::value;
-            fetch();
-            s2d::cp_async_wait<PF - 1>();
-            take(xn);
-            s2d::cascade<R, KIND, K, RN, WALL, PAR>(x.c, S, C, a.coin_last, a.ratio, a0 - K + i, a.em, jl, jr,
-                                                    [&](const cplx<R> (&o)[4][RN]) {
-                const bool row_ok = i >= 2 * K && i < nrows;                   // output row a0 + (i - 2K)
-                if (row_ok && st_lane && (!EDGE || st_full)) {
+        // the output row of input row i: a0 + (i - 2K)
+        auto put = [&](int i, const cplx<R> (&o)[4][RN]) {
+            const bool row_ok = i >= 2 * K && i < nrows;
+            if (row_ok && st_lane && (!EDGE || st_full)) {
+                char *o_ = op;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) { s2d::store_seg<RN>(reinterpret_cast<V *>(o_), o[c]); o_ += planeb; }
+            }
+            if constexpr (EDGE) {
+                if (row_ok && st_lane && !st_full) {
                     char *o_ = op;
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) { s2d::store_seg<RN>(reinterpret_cast<V *>(o_), o[c]); o_ += planeb; }
-                }
-                if constexpr (EDGE) {
-                    if (row_ok && st_lane && !st_full) {
-                        char *o_ = op;
+                    for (int c = 0; c < 4; ++c) {
 #pragma unroll
-                        for (int c = 0; c < 4; ++c) {
-#pragma unroll
-                            for (int j = 0; j < RN; ++j)
-                                if (col + j < a.en) cx_store<R>(reinterpret_cast<V *>(o_) + j, o[c][j]);
-                            o_ += planeb;
-                        }
+                        for (int j = 0; j < RN; ++j)
+                            if (col + j < a.en) cx_store<R>(reinterpret_cast<V *>(o_) + j, o[c][j]);
+                        o_ += planeb;
                     }
                 }
-                if (i >= 2 * K) op += rowb;
-            });
+            }
+            if (i >= 2 * K) op += rowb;
         };
 #pragma unroll 1
         for (int i = 0; i < PF; ++i) fetch();
         s2d::cp_async_wait<PF - 1>();
         s2d::Row<R, RN> xa, xb;
         take(xa);
+        if constexpr (S2dShape<R, K>::WAVE) {
+        // two input rows per trip, their cascades interleaved as a wavefront (s2d::cascade2)
+#pragma unroll 1
+        for (int i = 0; i < nrows; i += 2) {       // a surplus odd row is not stored
+            fetch();
+            fetch();
+            s2d::cp_async_wait<PF - 1>();
+            take(xb);
+            s2d::cascade2<R, KIND, K, RN, NS, WALL, 0>(xa.c, xb.c, S, c1s, C, a.coin_last, a.ratio, a0 - K + i, a.em, jl, jr,
+                                                   [&]() { take(xa); },
+                                                   [&](const cplx<R> (&o)[4][RN]) { put(i, o); },
+                                                   [&](const cplx<R> (&o)[4][RN]) { put(i + 1, o); });
+        }
+        } else {
+        // one cascade on x (input row i of the unit) while the row after it is taken from the ring into xn
+        auto one = [&](auto par_tag, int i, const s2d::Row<R, RN> &x, s2d::Row<R, RN> &xn) {
+            constexpr int PAR = decltype(par_tag)::value;
+            fetch();
+            s2d::cp_async_wait<PF - 1>();
+            take(xn);
+            s2d::cascade<R, KIND, K, RN, NS, WALL, PAR>(x.c, S, c1s, C, a.coin_last, a.ratio, a0 - K + i, a.em, jl, jr,
+                                                    [&](const cplx<R> (&o)[4][RN]) { put(i, o); });
+        };
 #pragma unroll 1
         for (int i = 0; i < nrows; i += 2) {       // always two cascades per trip (fixed register roles); a surplus odd row is not stored
             one(std::integral_constant<int, 0>{}, i, xa, xb);
             one(std::integral_constant<int, 1>{}, i + 1, xb, xa);
+        }
         }
         s2d::cp_async_wait<0>();
     };

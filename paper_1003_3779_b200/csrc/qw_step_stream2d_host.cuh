@@ -120,9 +120,11 @@ static int s2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
 template <typename R, int KIND>
 static int s2d_launch_kind(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
     switch (k) {
+#ifndef QW_S2D_DEV                    // (tuning builds compile the deep float instances of one coin only)
         case 2: return s2d_launch_k<R, KIND, 2>(s, in_buf, out_buf, box);
         case 4: return s2d_launch_k<R, KIND, 4>(s, in_buf, out_buf, box);
         case 6: return s2d_launch_k<R, KIND, 6>(s, in_buf, out_buf, box);
+#endif
         case 8: return s2d_launch_k<R, KIND, 8>(s, in_buf, out_buf, box);
         case 10: return s2d_launch_k<R, KIND, 10>(s, in_buf, out_buf, box);
         case 12: return s2d_launch_k<R, KIND, 12>(s, in_buf, out_buf, box);
@@ -133,8 +135,10 @@ static int s2d_launch_kind(qw_sim *s, int in_buf, int out_buf, int k, const Box 
 template <typename R>
 static int s2d_launch(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
     switch (s->coin_kind) {
+#ifndef QW_S2D_DEV
         case COIN_GROVER4: return s2d_launch_kind<R, COIN_GROVER4>(s, in_buf, out_buf, k, box);
         case COIN_HXH4:    return s2d_launch_kind<R, COIN_HXH4>(s, in_buf, out_buf, k, box);
+#endif
         case COIN_DFT4:    return s2d_launch_kind<R, COIN_DFT4>(s, in_buf, out_buf, k, box);
         default:           return s2d_launch_kind<R, COIN_GENERAL>(s, in_buf, out_buf, k, box);
     }

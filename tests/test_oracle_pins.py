@@ -508,6 +508,28 @@ def test_probabilities_marginalise_over_coin(oracle):
             assert abs(P[w, x] - want) <= 1e-17
 
 
+def test_probabilities_mean_is_the_batch_average(oracle):
+    """Pin of qwo_probabilities_mean (the ensemble average of the broken-links model): numpy's mean over
+    the walks of |psi|^2 summed over the coin (another routine, another order); closed forms: identical walks average to
+    the single walk, B delta states on B different sites give 1/B on each of them; the mean of normalised walks sums to 1."""
+    psi = qi.random_state(33, 5, 12, 4, normalise_per_walk=True)
+    got = oracle.probabilities_mean((3, 4), psi, batch=5)
+    want = np.mean(np.sum(psi.real ** 2 + psi.imag ** 2, axis=2), axis=0)
+    assert got.shape == (12,) and np.max(np.abs(got - want)) <= 1e-17
+    assert abs(np.sum(got) - 1.0) <= 1e-15
+    one = qi.random_state(34, 1, 9, 2)
+    rep = np.ascontiguousarray(np.repeat(one, 4, axis=0))
+    assert np.array_equal(oracle.probabilities_mean((9,), rep, batch=4), oracle.probabilities((9,), one)[0])
+    d = np.zeros((3, 7, 2), dtype=np.complex128)
+    for w, x in enumerate((1, 4, 6)):
+        d[w, x, w % 2] = 1j
+    got = oracle.probabilities_mean((7,), d, batch=3)
+    want = np.zeros(7); want[[1, 4, 6]] = 1.0 / 3.0
+    assert np.array_equal(got, want)
+    # a dropped walk, a transposed axis or a missing division fails one of the above; so does the wrong normalisation:
+    assert not np.allclose(got, np.sum(np.abs(d) ** 2, axis=(0, 2)))
+
+
 def test_sqrt_half_bit_patterns():
     import struct
     assert struct.pack("<d", qi.SQRT_HALF_F64) == struct.pack("<Q", 0x3FE6A09E667F3BCD)

@@ -398,13 +398,15 @@ def test_blocked_2d_delta_start_reaches_the_walls(qw, dev):
     assert np.array_equal(a[0], b[0])
 
 
+@pytest.mark.parametrize("kernel", [2, 1], ids=["stream", "tiles"])
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 @pytest.mark.parametrize("boundary", [qi.PERIODIC, qi.OPEN])
 @pytest.mark.parametrize("coin", ["grover", "hxh", "dft", "random"])
-def test_tiled_2d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, dtype, boundary, coin):
-    """P13 in 2D, register tiles: persistent CTAs advancing TMA-prefetched tiles k steps in registers
-    (renamed shifts, shuffles along n, shared-memory slots along m) == k fused single steps.
-    Extents span several tiles with ragged tails, fewer tiles than SMs, more tiles than SMs, odd widths."""
+def test_tiled_2d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, dtype, boundary, coin, kernel):
+    """P13 in 2D, state held in registers for k steps == k fused single steps, for both kernels of QW_SCHED_TILED:
+    the streaming kernel (warps streaming down strips of columns with a k-level pipeline of rows, shuffles along n, no
+    exchange along m) and the CTA tiles (TMA-prefetched tiles, renamed shifts, shuffles along n, shared-memory slots along m).
+    Extents span several tiles / strips with ragged tails, fewer units than SMs, more units than SMs, odd widths."""
     rng = np.random.default_rng(13)
     for extents, steps, k, batch in (((97, 130), 21, 0, 1), ((64, 64), 9, 2, 3), ((33, 200), 17, 4, 1),
                                      ((150, 41), 26, 6, 1), ((500, 700), 16, 8, 1), ((35, 32), 8, 8, 2)):
@@ -414,16 +416,57 @@ def test_tiled_2d_schedule_is_bit_identical_to_single_steps(qw, oracle, dev, dty
         w = qi.Workload("til2d", 2, extents, batch, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
                         state=qi.random_state(31, batch, sites, 4, dtype, normalise_per_walk=True))
         a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
-        b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k, options={qw.QW_OPT_TILED2D_KERNEL: kernel})
         assert b[3]["sched"] == qw.QW_SCHED_TILED
         assert np.array_equal(a[0], b[0]), (extents, steps, k)
         if sites < 20000:
             check_parity(w, b, oracle_run(oracle, w))
 
 
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.PERIODIC, qi.OPEN])
+def test_streaming_2d_kernel_depths_chains_and_edges(qw, oracle, dev, dtype, boundary):
+    """The streaming kernel beyond the shapes of the test above: its deepest pipelines (k = 10, 12 for complex64, 8 for
+    complex128), few warps (QW_OPT_MAX_CTAS) so that every warp runs many units one after the other and segments are cut
+    at many rows, lattices whose last strip holds one or two columns, a row count that is not a multiple of anything, odd
+    widths (a lane segment cut by the end of the row), batches; streaming == CTA tiles == fused steps bit for bit, and
+    parity with the oracle."""
+    rng = np.random.default_rng(17)
+    deep = (10, 12) if dtype == np.complex64 else (8, 6)
+    cases = [((211, 97), 27, deep[0], 1, 0), ((64, 49), 24, deep[1], 2, 1), ((301, 145), 20, 8, 1, 2),
+             ((73, 200), 31, 4, 3, 3), ((1000, 129), 16, 0, 1, 0)]
+    for extents, steps, k, batch, ctas in cases:
+        for coin in ("dft", "grover", "random"):
+            c = {"grover": qi.grover4, "dft": qi.dft4}[coin](dtype) if coin != "random" else qi.random_unitary(rng, 4).astype(dtype)
+            sites = extents[0] * extents[1]
+            w = qi.Workload("str2d", 2, extents, batch, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
+                            state=qi.random_state(37, batch, sites, 4, dtype, normalise_per_walk=True))
+            a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED)
+            b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k, options={qw.QW_OPT_TILED2D_KERNEL: 2, qw.QW_OPT_MAX_CTAS: ctas})
+            assert b[3]["sched"] == qw.QW_SCHED_TILED
+            assert np.array_equal(a[0], b[0]), (extents, steps, k, coin)
+            if k in (0, 2, 4, 6, 8):
+                t = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k, options={qw.QW_OPT_TILED2D_KERNEL: 1})
+                assert np.array_equal(t[0], b[0]), (extents, steps, k, coin)
+            if sites < 25000 and coin != "grover":
+                check_parity(w, b, oracle_run(oracle, w))
+    # a depth the kernel has no instance for
+    w = qi.k3(extents=(96, 80), steps=14, coin="dft", dtype=dtype)
+    h = qw.create_for(w)
+    try:
+        qw.load_state(h, w)
+        qw.qw_set_schedule(h, qw.QW_SCHED_TILED, 14)
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_step(h, 14)
+        assert ei.value.code == qw.QW_EINVAL
+    finally:
+        qw.qw_destroy(h)
+
+
+@pytest.mark.parametrize("kernel", [2, 1], ids=["stream", "tiles"])
 @pytest.mark.parametrize("window", [True, False])
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
-def test_tiled_2d_delta_start_reaches_the_walls(qw, dev, window, dtype):
+def test_tiled_2d_delta_start_reaches_the_walls(qw, dev, window, dtype, kernel):
     """Light-cone window on the tiled schedule (only tiles meeting the cone are launched) and the
     reflecting walls inside register tiles: the walker hits all four walls and comes back."""
     w = qi.k2(half=40, steps=131)
@@ -431,15 +474,16 @@ def test_tiled_2d_delta_start_reaches_the_walls(qw, dev, window, dtype):
     w.coin = w.coin.astype(dtype)
     w.delta_coin = w.delta_coin.astype(dtype)
     a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
+    opt = {qw.QW_OPT_TILED2D_KERNEL: kernel}
     for k in (0, 4):
-        b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k, window=window)
+        b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, k=k, window=window, options=opt)
         assert b[3]["sched"] == qw.QW_SCHED_TILED
         assert np.array_equal(a[0], b[0])
         assert np.array_equal(a[1], b[1])
     # off-centre start near a corner, walls met at different times
     w.delta_site = (3, 70)
     a = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
-    b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, window=window)
+    b = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, window=window, options=opt)
     assert np.array_equal(a[0], b[0])
 
 
@@ -545,10 +589,11 @@ def test_tiled_2d_diagonal_lattice_delta_start(qw, oracle, dev, dtype, boundary)
             qw.qw_destroy(h)
 
 
+@pytest.mark.parametrize("kernel", [2, 1], ids=["stream", "tiles"])
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 @pytest.mark.parametrize("coin", ["grover", "dft"])
-def test_light_cone_diamond_of_the_tiled_kernel(qw, oracle, dev, dtype, coin):
-    """The tiled 2D kernel skips every tile outside the cone's diamond |dm| + |dn| <= t (natural lattice).  Multi-tile
+def test_light_cone_diamond_of_the_tiled_kernel(qw, oracle, dev, dtype, coin, kernel):
+    """Both kernels of the tiled 2D schedule skip every tile / unit outside the cone's diamond |dm| + |dn| <= t (natural lattice).  Multi-tile
     lattices, off-centre starts: (a) open, the diamond is cut by two walls and reflects; (b) torus, the diamond is used
     until the cone's box wraps around, then switched off; (c) split stepping continues the same cone.  Window on ==
     window off bit for bit, and parity with the oracle."""
@@ -556,13 +601,14 @@ def test_light_cone_diamond_of_the_tiled_kernel(qw, oracle, dev, dtype, coin):
     dc = np.array([0.5, -0.5, -0.5, 0.5], dtype=dtype)
     for boundary, ext, site, steps in ((qi.OPEN, (150, 210), (20, 170), 120), (qi.PERIODIC, (97, 130), (48, 65), 70)):
         w = qi.Workload("dia", 2, ext, 1, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c, delta_site=site, delta_coin=dc)
-        on = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, window=True)
+        on = gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, window=True, options={qw.QW_OPT_TILED2D_KERNEL: kernel})
         off = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
         assert on[3]["sched"] == qw.QW_SCHED_TILED
         assert np.array_equal(on[0], off[0]), (boundary, ext)
         check_parity(w, on, oracle_run(oracle, w))
         h = qw.create_for(w)
         try:
+            qw.qw_set_option(h, qw.QW_OPT_TILED2D_KERNEL, kernel)
             qw.qw_set_schedule(h, qw.QW_SCHED_TILED, 0)
             qw.load_state(h, w)
             qw.qw_step(h, 13); qw.qw_step(h, steps - 13)

@@ -191,3 +191,44 @@ def test_rbl_2d_even_rows_share_generator_calls_between_lane_pairs(qw, oracle, d
         gen = gpu_rbl(qw, w, 0.2, SEED, steps, schedule=qw.QW_SCHED_GENERIC, window=False)
         assert np.array_equal(on[0], off[0]) and np.array_equal(off[0], gen[0]), (ext, site)
         close(w, on[0], psi)
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("dim", [1, 2])
+def test_ensemble_average_over_the_batch(qw, oracle, dev, dtype, dim):
+    """qw_probabilities_mean (SURVEY.md 8(f) NEXT-2 "ensemble averages over the batch axis"): a batch of walks from ONE initial
+    state, every walk with its own random broken links, averaged per site — against the oracle's
+    average of the oracle's walks; host and device output buffers; odd row lengths; p = 0 gives the single walk back."""
+    import torch
+    batch = 24
+    ext = (4099,) if dim == 1 else (37, 75)
+    sites = int(np.prod(ext))
+    one = qi.random_state(41, 1, sites, 2 * dim, dtype)
+    state = np.ascontiguousarray(np.repeat(one, batch, axis=0))
+    coin = qi.hadamard(dtype) if dim == 1 else qi.grover4(dtype)
+    w = qi.Workload("ens", dim, ext, batch, qi.PERIODIC, np.dtype(dtype), 12, qi.COIN_UNIFORM, coin, state=state)
+    rt = np.float64 if dtype == np.complex128 else np.float32
+    tol = 1e-12 if dtype == np.complex128 else 1e-7
+    for p in (0.25, 0.0):
+        h = qw.create_for(w)
+        try:
+            qw.qw_set_random_broken_links(h, 1, p, SEED)
+            qw.load_state(h, w)
+            qw.qw_step(h, w.steps)
+            host = np.empty((sites,), dtype=rt)
+            qw.qw_probabilities_mean(h, host)
+            devbuf = torch.empty((sites,), dtype=torch.float64 if rt == np.float64 else torch.float32, device=dev)
+            qw.qw_probabilities_mean(h, devbuf)
+            P = np.empty((batch, sites), dtype=rt)
+            qw.qw_probabilities(h, P)
+        finally:
+            qw.qw_destroy(h)
+        assert np.array_equal(host, devbuf.cpu().numpy())
+        psi = oracle_rbl(oracle, w, p, SEED, w.steps)
+        want = oracle.probabilities_mean(ext, psi, batch=batch)
+        assert float(np.max(np.abs(host.astype(np.float64) - want))) <= tol
+        assert abs(float(np.sum(host.astype(np.float64))) - 1.0) <= (1e-12 if dtype == np.complex128 else 1e-4)
+        if p == 0.0:          # no broken links: all walks are the same walk
+            assert float(np.max(np.abs(host.astype(np.float64) - P[0].astype(np.float64)))) <= tol
+        else:                 # the realisations differ, the average is none of them
+            assert float(np.max(np.abs(P[0].astype(np.float64) - P[1].astype(np.float64)))) > 1e-6
