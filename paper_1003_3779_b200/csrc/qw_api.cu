@@ -451,7 +451,7 @@ int qw_step(qw_sim *s, int64_t n) {
         sched = resident1d_eligible(s) ? QW_SCHED_RESIDENT
               : ((blocked1d_eligible(s) && n >= 4) ||
                  (chain1d_eligible(s, chain1d_granule(s)) && n >= chain1d_granule(s))) ? QW_SCHED_BLOCKED
-              : (tiled2d_eligible(s) && n >= 2) ? QW_SCHED_TILED : QW_SCHED_FUSED;
+              : ((tiled2d_eligible(s) || stream2d_eligible(s)) && n >= 2) ? QW_SCHED_TILED : QW_SCHED_FUSED;
     if (sched == QW_SCHED_RESIDENT) {
         if (!resident1d_eligible(s))
             return fail(QW_EUNSUPPORTED, "the resident schedule needs 1D walks of at most 4096 sites, no per-site matrices, no link mask");
@@ -465,18 +465,19 @@ int qw_step(qw_sim *s, int64_t n) {
         return fail(QW_EUNSUPPORTED, "the temporally blocked schedule needs a uniform coin without phases or link mask on a 1D "
                                      "lattice of >= %d sites or a natural 2D lattice of >= 32 x 32 sites",
                     32 * blocked1d_granule(s));
-    if (sched == QW_SCHED_TILED && !tiled2d_eligible(s))
+    if (sched == QW_SCHED_TILED && !tiled2d_eligible(s) && !stream2d_eligible(s))
         return fail(QW_EUNSUPPORTED, "the tiled schedule needs a uniform coin without phases or link mask on a 2D lattice of "
                                      ">= 32 x 32 sites (diagonal lattice: a torus, or an open lattice with a delta start)");
-    const bool stream2d = sched == QW_SCHED_TILED && s->tiled2d_kernel != 1 && stream2d_eligible(s);
+    // natural lattice: the streaming kernel unless the CTA tiles are asked for (which have no instance with link draws)
+    const bool stream2d = sched == QW_SCHED_TILED && stream2d_eligible(s) && (s->tiled2d_kernel != 1 || !tiled2d_eligible(s));
     if (sched == QW_SCHED_TILED && (s->sched_k < 0 || s->sched_k % 2 != 0 || s->sched_k > (stream2d ? stream2d_max_k(s) : 8)))
         return fail(QW_EINVAL, "the tiled schedule takes an even k <= %d here (got %d)", stream2d ? stream2d_max_k(s) : 8, s->sched_k);
     int64_t remaining = n;
     s->last_sched = sched; s->last_k = 1;
     if (sched == QW_SCHED_TILED) {
         // k-step launches, then the even part of the remainder; an odd last step goes through the fused kernel below
-        // measured optima on B200 (profiles/), both kernels: 8 (complex64) / 6 (complex128)
-        const int kmax = s->sched_k > 0 ? s->sched_k : (s->dtype == QW_C128 ? 6 : 8);
+        // measured optima on B200 (profiles/), both kernels: 8 (complex64) / 6 (complex128); with link draws 6 (registers)
+        const int kmax = s->sched_k > 0 ? s->sched_k : ((s->dtype == QW_C128 || s->rbl) ? 6 : 8);
         s->last_k = kmax;
         while (remaining >= 2) {
             const int kk = (int)(remaining >= kmax ? kmax : remaining / 2 * 2);

@@ -190,6 +190,8 @@ int stream2d_max_k(const qw_sim *s);
 int launch_step_stream2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 int launch_stream2d_f32(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 int launch_stream2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
+int launch_stream2d_rbl_f32(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);   // random broken links drawn in the kernel
+int launch_stream2d_rbl_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 
 // qw_reduce.cu
 int launch_probabilities(qw_sim *s, const void *state, void *out_dev);

@@ -320,14 +320,22 @@ int launch_step_tiled2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &bo
 }
 
 // Streaming schedule (qw_step_stream2d.cuh): natural lattice, uniform coin; same ghost ring as the tiles.
-bool stream2d_eligible(const qw_sim *s) { return blocked2d_eligible(s); }
-int stream2d_max_k(const qw_sim *s) { return s->dtype == QW_C128 ? 8 : 12; }
+// Random broken links redrawn every step are drawn inside the kernel when the rows have even length (two sites of a
+// lane share one generator call); depth <= 8 then.
+bool stream2d_eligible(const qw_sim *s) {
+    const Geom &g = s->g;
+    return g.dim == 2 && g.lattice == QW_NATURAL && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
+           (!s->rbl || g.en % 2 == 0) && g.em >= 2 * QW_GHOST_2D && g.en >= 2 * QW_GHOST_2D && g.batch <= 16383 &&
+           g.walk_stride * 4 * g.batch < (1LL << 40);
+}
+int stream2d_max_k(const qw_sim *s) { return (s->dtype == QW_C128 || s->rbl) ? 8 : 12; }
 
 int launch_step_stream2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
     if (s->g.boundary == QW_PERIODIC) {
         int rc = launch_ghost_refresh(s, in_buf);
         if (rc) return rc;
     }
+    if (s->rbl) return s->dtype == QW_C128 ? launch_stream2d_rbl_f64(s, in_buf, out_buf, k, box) : launch_stream2d_rbl_f32(s, in_buf, out_buf, k, box);
     return s->dtype == QW_C128 ? launch_stream2d_f64(s, in_buf, out_buf, k, box) : launch_stream2d_f32(s, in_buf, out_buf, k, box);
 }
 

@@ -29,6 +29,7 @@
 #include <type_traits>
 
 #include "qw_coin.cuh"
+#include "qw_philox.cuh"
 
 #ifndef QW_S2D_WAVE
 #define QW_S2D_WAVE 0
@@ -40,20 +41,20 @@ namespace qw {
 // whole number of 16-byte vectors), WPC = warps per CTA (one CTA per SM; 12 warps leave 168 registers per thread, 8 leave
 // 255 — the pipeline holds 4*RN complex amplitudes per level), RING / PF = rows of the per-warp input ring in shared
 // memory / prefetch distance (WPC * RING * 4 * 32*RN * sizeof(complex) <= 192 KiB).
-template <typename R, int K> struct S2dShape;
+template <typename R, int K, bool RBL = false> struct S2dShape;
 // NS = number of levels (the first NS) whose two parked phi_1 rows live in shared memory instead of registers (one 16-byte
 // load and store per level and row): what lets the deep pipelines fit the register file.
 #ifndef QW_S2D_NS10
 #define QW_S2D_NS10 5
 #define QW_S2D_NS12 8
 #endif
-template <int K> struct S2dShape<float, K> {
-    static constexpr int RN = 2, WPC = (K <= 4) ? 12 : 8, RING = 8, PF = 6;
+template <int K, bool RBL> struct S2dShape<float, K, RBL> {      // (link draws cost ~25 registers: 8 warps from k = 4 on)
+    static constexpr int RN = 2, WPC = (K <= (RBL ? 2 : 4)) ? 12 : 8, RING = 8, PF = 6;
     static constexpr int NS = K <= 8 ? 0 : (K == 10 ? QW_S2D_NS10 : QW_S2D_NS12);
     static constexpr bool WAVE = QW_S2D_WAVE != 0;
 };
-template <int K> struct S2dShape<double, K> {
-    static constexpr int RN = (K <= 4) ? 2 : 1, WPC = (K <= 2) ? 12 : 8, RING = (K <= 4) ? 4 : 8, PF = RING - 1;
+template <int K, bool RBL> struct S2dShape<double, K, RBL> {
+    static constexpr int RN = (K <= 4) ? 2 : 1, WPC = (K <= (RBL ? 0 : 2)) ? 12 : 8, RING = (K <= 4) ? 4 : 8, PF = RING - 1;
     static constexpr int NS = 0;
     static constexpr bool WAVE = QW_S2D_WAVE != 0;
 };
@@ -74,6 +75,10 @@ struct Stream2dArgs {
     R coin_last[32];              // deferred scale of the named coins: coin * scale^(K-1) (qw_coin.cuh: apply_coin_bare)
     R ratio;                      // Grover-like: (d - g) / g
     long long dia_m, dia_n, dia_r;   // light-cone diamond (dia_r < 0: none), as in qw_step_tiled2d.cuh
+    // random broken links (RBL instances): link number = owner * 2 + axis is broken at step t iff
+    // philox4x32_10(counter = (number / 4 lo, hi, t, walk), key)[number mod 4] < rbl_thr
+    unsigned rbl_key0, rbl_key1, t;
+    unsigned long long rbl_thr;
 };
 
 namespace s2d {
@@ -169,13 +174,57 @@ __device__ __forceinline__ cplx<R> coin_back(const cplx<R> (&t)[4]) {
 // the back stage of level l produces phi_0, phi_1, phi_3 — straight into those registers.
 // WALL: r = the input row as a row of the lattice (rows 0 / em-1 are walls), jl / jr = this lane's local column of
 // lattice column 0 / en-1 (or -1).
+// What a warp carries through the cascades of one unit besides the pipeline itself.
+template <typename R>
+struct Ctx {
+    const R *C, *Clast;           // coin; coin * scale^(K-1) for the last level (deferred scale)
+    R ratio;
+    long long em, en;
+    int jl, jr;                   // this lane's local column of lattice column 0 / en-1 (walls), or -1
+    // random broken links (eqs. 9-10; R27), RBL instances only
+    long long colw;               // this lane's first column as a column of the lattice (wrapped on a torus)
+    unsigned k0, k1, t0, walk;    // generator key, step index of level 0, walk index
+    unsigned long long thr;       // a link is broken iff its 32-bit draw is below thr
+    unsigned mbits;               // per level and column: is the link to the row BELOW the last coined row broken (bit L*RN + j)
+};
+
 // ---- one level boundary of a cascade: t = front-stage values of the row (lattice row q) that level L is coining
 // c1s != nullptr: the two parked phi_1 rows of this level live in shared memory, c1s[parity][lane][RN] (this lane's entry).
-template <typename R, int KIND, int K, int RN, bool WALL, int PAR, int L, bool C1S, typename Emit>
-__device__ __forceinline__ void level_step(cplx<R> (&t)[RN][4], Level<R, RN> &S, typename Cx<R>::T *c1s, const R *C, const R *Clast,
-                                           R ratio, long long q, long long em, int jl, int jr, Emit emit) {
+// RBL: every link is redrawn at every step (level L = step t0 + L).  One generator call yields the four links the lane's
+// two sites own (reading R27: number = owner * 2 + axis, four consecutive numbers per call); a broken link along n keeps
+// phi_0 / phi_3 on their sites with the opposite coin — for the link to the next lane the owner's bit travels with one
+// more shuffle —, a broken link along m is the swap (phi_2 of this row <-> parked phi_1 of the row above) one cascade
+// later, when the row below is coined: the bits wait in cx.mbits.
+template <typename R, int KIND, int K, int RN, bool WALL, bool RBL, int PAR, int L, bool C1S, typename Emit>
+__device__ __forceinline__ void level_step(cplx<R> (&t)[RN][4], Level<R, RN> &S, typename Cx<R>::T *c1s, Ctx<R> &cx, long long q,
+                                           Emit emit) {
     constexpr int C1P = 32 * RN;                        // elements between the two parities
     if constexpr (C1S) load_seg<RN>(c1s + PAR * C1P, S.c1[PAR]);
+    bool bn[RN], bm[RN];                                // links owned by the sites of row q: along n (to column +1), along m (to row +1)
+    if constexpr (RBL) {
+        long long qq = q;                               // the row as a row of the lattice
+        if constexpr (!WALL) { if (qq < 0) qq += cx.em; else if (qq >= cx.em) qq -= cx.em; }
+        const unsigned long long owner = (unsigned long long)(qq * cx.en + cx.colw);
+        unsigned w[4];
+        if constexpr (RN == 2) {                        // even row length, even column: the two sites share one call
+            rbl_group_words(owner >> 1, cx.t0 + L, cx.walk, cx.k0, cx.k1, w);
+            bn[0] = w[0] < cx.thr; bm[0] = w[1] < cx.thr; bn[1] = w[2] < cx.thr; bm[1] = w[3] < cx.thr;
+        } else {
+            static_assert(RN == 1 || RN == 2, "link draws are written for one or two sites per lane");
+            rbl_group_words(owner >> 1, cx.t0 + L, cx.walk, cx.k0, cx.k1, w);
+            const bool odd = (owner & 1ull) != 0;
+            bn[0] = (odd ? w[2] : w[0]) < cx.thr; bm[0] = (odd ? w[3] : w[1]) < cx.thr;
+        }
+        if constexpr (WALL) {                           // links that leave the lattice belong to the wall code
+#pragma unroll
+            for (int j = 0; j < RN; ++j) {
+                const long long cj = cx.colw + j;
+                const bool in = qq >= 0 && qq < cx.em && cj >= 0 && cj < cx.en;
+                bn[j] = bn[j] && in && cj < cx.en - 1;
+                bm[j] = bm[j] && in && qq < cx.em - 1;
+            }
+        }
+    }
     // ---- phi_2 of row q completes row q-1 of level L+1
     cplx<R> c2n[RN];
 #pragma unroll
@@ -184,18 +233,37 @@ __device__ __forceinline__ void level_step(cplx<R> (&t)[RN][4], Level<R, RN> &S,
     if constexpr (WALL) {
 #pragma unroll
         for (int j = 0; j < RN; ++j) y2w[j] = c2n[j];
-        if (q == em) {                                 // bottom wall: phi_1 of row em-1 (parked for row em) -> c2 of row em-1
+        if (q == cx.em) {                              // bottom wall: phi_1 of row em-1 (parked for row em) -> c2 of row em-1
             if constexpr (C1S) load_seg<RN>(c1s + (PAR ^ 1) * C1P, S.c1[PAR ^ 1]);
 #pragma unroll
             for (int j = 0; j < RN; ++j) c2n[j] = S.c1[PAR ^ 1][j];
         }
+    }
+    if constexpr (RBL) {
+        // links between rows q-1 and q (drawn one cascade ago): broken = phi_1 of row q-1 and phi_2 of row q stay where they are
+        const unsigned prev = cx.mbits >> (L * RN);
+        if constexpr (C1S) { if (prev & ((1u << RN) - 1u)) load_seg<RN>(c1s + (PAR ^ 1) * C1P, S.c1[PAR ^ 1]); }
+        bool any = false;
+#pragma unroll
+        for (int j = 0; j < RN; ++j) {
+            const bool b = (prev >> j) & 1u;
+            const cplx<R> up = c2n[j], parked = S.c1[PAR ^ 1][j];
+            c2n[j] = b ? parked : up;
+            S.c1[PAR ^ 1][j] = b ? up : parked;
+            any = any || b;
+        }
+        if constexpr (C1S) { if (any) store_seg<RN>(c1s + (PAR ^ 1) * C1P, S.c1[PAR ^ 1]); }
+        unsigned nb = 0;
+#pragma unroll
+        for (int j = 0; j < RN; ++j) nb |= (bm[j] ? 1u : 0u) << j;
+        cx.mbits = (cx.mbits & ~(((1u << RN) - 1u) << (L * RN))) | (nb << (L * RN));
     }
     cplx<R> tn[RN][4];
     if constexpr (L + 1 < K) {
 #pragma unroll
         for (int j = 0; j < RN; ++j) {
             const cplx<R> v[4] = {S.c0[j], S.c1[PAR][j], c2n[j], S.c3[j]};
-            coin_front<R, KIND, L + 2 == K>(C, Clast, ratio, v, tn[j]);
+            coin_front<R, KIND, L + 2 == K>(cx.C, cx.Clast, cx.ratio, v, tn[j]);
         }
     } else {
         cplx<R> out[4][RN];
@@ -214,12 +282,22 @@ __device__ __forceinline__ void level_step(cplx<R> (&t)[RN][4], Level<R, RN> &S,
     S.c3[RN - 1] = shfl_down1(y3[0]);                  // phi_3 of the lane to the right enters column RN-1
 #pragma unroll
     for (int j = 1; j < RN; ++j) { S.c0[j] = y0[j - 1]; S.c3[j - 1] = y3[j]; }
+    if constexpr (RBL) {
+        // broken links along n: both ends keep their outgoing component with the opposite coin
+        const bool bl = __shfl_up_sync(0xffffffffu, bn[RN - 1] ? 1 : 0, 1) != 0;   // the link owned by the lane to the left
+        if (bl) S.c0[0] = y3[0];
+        if (bn[RN - 1]) S.c3[RN - 1] = y0[RN - 1];
+#pragma unroll
+        for (int j = 1; j < RN; ++j) {
+            if (bn[j - 1]) { S.c0[j] = y3[j]; S.c3[j - 1] = y0[j - 1]; }
+        }
+    }
     if constexpr (WALL) {
         // reflecting walls (RBL = 0): the outgoing component stays with the opposite coin
 #pragma unroll
         for (int j = 0; j < RN; ++j) {
-            if (jl == j) S.c0[j] = y3[j];              // left wall:  phi_3 -> c0 of the same site
-            if (jr == j) S.c3[j] = y0[j];              // right wall: phi_0 -> c3 of the same site
+            if (cx.jl == j) S.c0[j] = y3[j];           // left wall:  phi_3 -> c0 of the same site
+            if (cx.jr == j) S.c3[j] = y0[j];           // right wall: phi_0 -> c3 of the same site
         }
         if (q == 0) {                                  // top wall: phi_2 -> c1 of row 0 (instead of phi_1 of row -1)
 #pragma unroll
@@ -237,11 +315,11 @@ __device__ __forceinline__ void level_step(cplx<R> (&t)[RN][4], Level<R, RN> &S,
 }
 
 template <typename R, int KIND, int K, int RN>
-__device__ __forceinline__ void front0(const cplx<R> (&x)[4][RN], cplx<R> (&t)[RN][4], const R *C, const R *Clast, R ratio) {
+__device__ __forceinline__ void front0(const cplx<R> (&x)[4][RN], cplx<R> (&t)[RN][4], const Ctx<R> &cx) {
 #pragma unroll
     for (int j = 0; j < RN; ++j) {
         const cplx<R> v[4] = {x[0][j], x[1][j], x[2][j], x[3][j]};
-        coin_front<R, KIND, K == 1>(C, Clast, ratio, v, t[j]);
+        coin_front<R, KIND, K == 1>(cx.C, cx.Clast, cx.ratio, v, t[j]);
     }
 }
 
@@ -250,66 +328,67 @@ template <typename R, int RN, int NS, int L> __device__ __forceinline__ typename
     return L < NS ? c1s + L * 2 * 32 * RN : nullptr;
 }
 
-template <typename R, int KIND, int K, int RN, int NS, bool WALL, int PAR, int L, typename Emit>
+// One cascade: input row r (complete, in x) passes level 0, the row it completes passes level 1, ...; emit(out) is called
+// with row r-K of level K.  PAR = parity of the cascade count (which of the two phi_1 slots is due).
+// Order inside a level boundary (what keeps the register allocation free of moves): phi_2 of level l first; with it the
+// completed row of level l+1 goes through ITS front stage, which is the last reader of the parked registers; only then
+// the back stage of level l produces phi_0, phi_1, phi_3 — straight into those registers.
+// WALL: r = the input row as a row of the lattice (rows 0 / em-1 are walls).
+template <typename R, int KIND, int K, int RN, int NS, bool WALL, bool RBL, int PAR, int L, typename Emit>
 struct Levels {
-    static __device__ __forceinline__ void run(cplx<R> (&t)[RN][4], Level<R, RN> (&S)[K], typename Cx<R>::T *c1s, const R *C,
-                                               const R *Clast, R ratio, long long r, long long em, int jl, int jr, Emit emit) {
-        level_step<R, KIND, K, RN, WALL, PAR, L, (L < NS)>(t, S[L], c1_of<R, RN, NS, L>(c1s), C, Clast, ratio, r - L, em, jl, jr, emit);
-        if constexpr (L + 1 < K) Levels<R, KIND, K, RN, NS, WALL, PAR, L + 1, Emit>::run(t, S, c1s, C, Clast, ratio, r, em, jl, jr, emit);
+    static __device__ __forceinline__ void run(cplx<R> (&t)[RN][4], Level<R, RN> (&S)[K], typename Cx<R>::T *c1s, Ctx<R> &cx,
+                                               long long r, Emit emit) {
+        level_step<R, KIND, K, RN, WALL, RBL, PAR, L, (L < NS)>(t, S[L], c1_of<R, RN, NS, L>(c1s), cx, r - L, emit);
+        if constexpr (L + 1 < K) Levels<R, KIND, K, RN, NS, WALL, RBL, PAR, L + 1, Emit>::run(t, S, c1s, cx, r, emit);
     }
 };
-template <typename R, int KIND, int K, int RN, int NS, bool WALL, int PAR, typename Emit>
-__device__ __forceinline__ void cascade(const cplx<R> (&x)[4][RN], Level<R, RN> (&S)[K], typename Cx<R>::T *c1s, const R *C,
-                                        const R *Clast, R ratio, long long r, long long em, int jl, int jr, Emit emit) {
+template <typename R, int KIND, int K, int RN, int NS, bool WALL, bool RBL, int PAR, typename Emit>
+__device__ __forceinline__ void cascade(const cplx<R> (&x)[4][RN], Level<R, RN> (&S)[K], typename Cx<R>::T *c1s, Ctx<R> &cx,
+                                        long long r, Emit emit) {
     cplx<R> t[RN][4];
-    front0<R, KIND, K, RN>(x, t, C, Clast, ratio);
-    Levels<R, KIND, K, RN, NS, WALL, PAR, 0, Emit>::run(t, S, c1s, C, Clast, ratio, r, em, jl, jr, emit);
+    front0<R, KIND, K, RN>(x, t, cx);
+    Levels<R, KIND, K, RN, NS, WALL, RBL, PAR, 0, Emit>::run(t, S, c1s, cx, r, emit);
 }
 
 // Two cascades as a wavefront: row r (parity PAR) runs one level ahead of row r+1 (parity PAR^1), so that at any
 // time two independent dependency chains are in flight in the warp.  Level L of row r+1 reads what level L of row r
 // has parked in the step before: the same order of updates as two cascades one after the other.
-template <typename R, int KIND, int K, int RN, int NS, bool WALL, int PAR, int L, typename EmitA, typename EmitB>
+template <typename R, int KIND, int K, int RN, int NS, bool WALL, bool RBL, int PAR, int L, typename EmitA, typename EmitB>
 struct Wave {
     static __device__ __forceinline__ void run(cplx<R> (&ta)[RN][4], cplx<R> (&tb)[RN][4], Level<R, RN> (&S)[K], typename Cx<R>::T *c1s,
-                                               const R *C, const R *Clast, R ratio, long long r, long long em, int jl, int jr,
-                                               EmitA ea, EmitB eb) {
-        level_step<R, KIND, K, RN, WALL, PAR, L, (L < NS)>(ta, S[L], c1_of<R, RN, NS, L>(c1s), C, Clast, ratio, r - L, em, jl, jr, ea);
-        level_step<R, KIND, K, RN, WALL, PAR ^ 1, L - 1, (L - 1 < NS)>(tb, S[L - 1], c1_of<R, RN, NS, L - 1>(c1s), C, Clast, ratio,
-                                                                      r + 1 - (L - 1), em, jl, jr, eb);
-        if constexpr (L + 1 < K)
-            Wave<R, KIND, K, RN, NS, WALL, PAR, L + 1, EmitA, EmitB>::run(ta, tb, S, c1s, C, Clast, ratio, r, em, jl, jr, ea, eb);
+                                               Ctx<R> &cx, long long r, EmitA ea, EmitB eb) {
+        level_step<R, KIND, K, RN, WALL, RBL, PAR, L, (L < NS)>(ta, S[L], c1_of<R, RN, NS, L>(c1s), cx, r - L, ea);
+        level_step<R, KIND, K, RN, WALL, RBL, PAR ^ 1, L - 1, (L - 1 < NS)>(tb, S[L - 1], c1_of<R, RN, NS, L - 1>(c1s), cx, r + 1 - (L - 1), eb);
+        if constexpr (L + 1 < K) Wave<R, KIND, K, RN, NS, WALL, RBL, PAR, L + 1, EmitA, EmitB>::run(ta, tb, S, c1s, cx, r, ea, eb);
     }
 };
 // mid() is called as soon as xa has been read for the last time (the caller refills it with the row after next).
-template <typename R, int KIND, int K, int RN, int NS, bool WALL, int PAR, typename Mid, typename EmitA, typename EmitB>
+template <typename R, int KIND, int K, int RN, int NS, bool WALL, bool RBL, int PAR, typename Mid, typename EmitA, typename EmitB>
 __device__ __forceinline__ void cascade2(const cplx<R> (&xa)[4][RN], const cplx<R> (&xb)[4][RN], Level<R, RN> (&S)[K],
-                                         typename Cx<R>::T *c1s, const R *C, const R *Clast, R ratio, long long r, long long em,
-                                         int jl, int jr, Mid mid, EmitA ea, EmitB eb) {
+                                         typename Cx<R>::T *c1s, Ctx<R> &cx, long long r, Mid mid, EmitA ea, EmitB eb) {
     static_assert(K >= 2, "the wavefront needs two levels");
     cplx<R> ta[RN][4], tb[RN][4];
-    front0<R, KIND, K, RN>(xa, ta, C, Clast, ratio);
+    front0<R, KIND, K, RN>(xa, ta, cx);
     mid();
-    level_step<R, KIND, K, RN, WALL, PAR, 0, (0 < NS)>(ta, S[0], c1_of<R, RN, NS, 0>(c1s), C, Clast, ratio, r, em, jl, jr, ea);
-    front0<R, KIND, K, RN>(xb, tb, C, Clast, ratio);
-    Wave<R, KIND, K, RN, NS, WALL, PAR, 1, EmitA, EmitB>::run(ta, tb, S, c1s, C, Clast, ratio, r, em, jl, jr, ea, eb);
-    level_step<R, KIND, K, RN, WALL, PAR ^ 1, K - 1, (K - 1 < NS)>(tb, S[K - 1], c1_of<R, RN, NS, K - 1>(c1s), C, Clast, ratio,
-                                                                  r + 1 - (K - 1), em, jl, jr, eb);
+    level_step<R, KIND, K, RN, WALL, RBL, PAR, 0, (0 < NS)>(ta, S[0], c1_of<R, RN, NS, 0>(c1s), cx, r, ea);
+    front0<R, KIND, K, RN>(xb, tb, cx);
+    Wave<R, KIND, K, RN, NS, WALL, RBL, PAR, 1, EmitA, EmitB>::run(ta, tb, S, c1s, cx, r, ea, eb);
+    level_step<R, KIND, K, RN, WALL, RBL, PAR ^ 1, K - 1, (K - 1 < NS)>(tb, S[K - 1], c1_of<R, RN, NS, K - 1>(c1s), cx, r + 1 - (K - 1), eb);
 }
 
 }  // namespace s2d
 
-template <typename R, int K> constexpr size_t stream2d_smem_bytes() {
-    return (size_t)S2dShape<R, K>::WPC * (S2dShape<R, K>::RING * 4 + S2dShape<R, K>::NS * 2) * (32 * S2dShape<R, K>::RN) *
+template <typename R, int K, bool RBL> constexpr size_t stream2d_smem_bytes() {
+    return (size_t)S2dShape<R, K, RBL>::WPC * (S2dShape<R, K, RBL>::RING * 4 + S2dShape<R, K, RBL>::NS * 2) * (32 * S2dShape<R, K, RBL>::RN) *
            sizeof(typename Cx<R>::T);
 }
 
-template <typename R, int KIND, bool OPEN, int K>
-__global__ void __launch_bounds__(S2dShape<R, K>::WPC * 32, 1)
+template <typename R, int KIND, bool OPEN, int K, bool RBL = false>
+__global__ void __launch_bounds__(S2dShape<R, K, RBL>::WPC * 32, 1)
 step_stream2d_kernel(const Stream2dArgs<R> a) {
     typedef typename Cx<R>::T V;
-    constexpr int RN = S2dShape<R, K>::RN, HN = 32 * RN, VN = HN - 2 * K;
-    constexpr int WPC = S2dShape<R, K>::WPC, RING = S2dShape<R, K>::RING, PF = S2dShape<R, K>::PF, NS = S2dShape<R, K>::NS;
+    constexpr int RN = S2dShape<R, K, RBL>::RN, HN = 32 * RN, VN = HN - 2 * K;
+    constexpr int WPC = S2dShape<R, K, RBL>::WPC, RING = S2dShape<R, K, RBL>::RING, PF = S2dShape<R, K, RBL>::PF, NS = S2dShape<R, K, RBL>::NS;
     static_assert(VN > 0, "block depth too large for the strip");
     static_assert(sizeof(V) == 16 || K % 2 == 0, "complex64 strips need an even halo (16-byte aligned lane segments)");
     static_assert(K % RN == 0, "the halo must be a whole number of lane segments");
@@ -339,7 +418,14 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
         const long long planeb = a.plane_stride * (long long)sizeof(V);
         const long long rowb = a.pitch * (long long)sizeof(V);
         const long long jl_ = -col, jr_ = a.en - 1 - col;
-        const int jl = (jl_ >= 0 && jl_ < RN) ? (int)jl_ : -1, jr = (jr_ >= 0 && jr_ < RN) ? (int)jr_ : -1;
+        s2d::Ctx<R> cx;
+        cx.C = C; cx.Clast = a.coin_last; cx.ratio = a.ratio; cx.em = a.em; cx.en = a.en;
+        cx.jl = (jl_ >= 0 && jl_ < RN) ? (int)jl_ : -1; cx.jr = (jr_ >= 0 && jr_ < RN) ? (int)jr_ : -1;
+        if constexpr (RBL) {
+            cx.colw = col;
+            if constexpr (!OPEN) { if (cx.colw < 0) cx.colw += a.en; else if (cx.colw >= a.en) cx.colw -= a.en; }
+            cx.k0 = a.rbl_key0; cx.k1 = a.rbl_key1; cx.t0 = a.t; cx.walk = (unsigned)w; cx.thr = a.rbl_thr; cx.mbits = 0;
+        }
         const bool st_lane = (lane * RN >= K) && (lane * RN + RN <= HN - K) && col < a.en;
         const bool st_full = col + RN <= a.en;                                 // always true in a unit that is not EDGE
         const int nrows = (int)(b0 - a0) + 2 * K;
@@ -404,7 +490,7 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
         s2d::cp_async_wait<PF - 1>();
         s2d::Row<R, RN> xa, xb;
         take(xa);
-        if constexpr (S2dShape<R, K>::WAVE) {
+        if constexpr (S2dShape<R, K, RBL>::WAVE) {
         // two input rows per trip, their cascades interleaved as a wavefront (s2d::cascade2)
 #pragma unroll 1
         for (int i = 0; i < nrows; i += 2) {       // a surplus odd row is not stored
@@ -412,7 +498,7 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
             fetch();
             s2d::cp_async_wait<PF - 1>();
             take(xb);
-            s2d::cascade2<R, KIND, K, RN, NS, WALL, 0>(xa.c, xb.c, S, c1s, C, a.coin_last, a.ratio, a0 - K + i, a.em, jl, jr,
+            s2d::cascade2<R, KIND, K, RN, NS, WALL, RBL, 0>(xa.c, xb.c, S, c1s, cx, a0 - K + i,
                                                    [&]() { take(xa); },
                                                    [&](const cplx<R> (&o)[4][RN]) { put(i, o); },
                                                    [&](const cplx<R> (&o)[4][RN]) { put(i + 1, o); });
@@ -424,7 +510,7 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
             fetch();
             s2d::cp_async_wait<PF - 1>();
             take(xn);
-            s2d::cascade<R, KIND, K, RN, NS, WALL, PAR>(x.c, S, c1s, C, a.coin_last, a.ratio, a0 - K + i, a.em, jl, jr,
+            s2d::cascade<R, KIND, K, RN, NS, WALL, RBL, PAR>(x.c, S, c1s, cx, a0 - K + i,
                                                     [&](const cplx<R> (&o)[4][RN]) { put(i, o); });
         };
 #pragma unroll 1

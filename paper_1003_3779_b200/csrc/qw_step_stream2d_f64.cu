@@ -2,5 +2,5 @@
 #include "qw_step_stream2d_host.cuh"
 
 namespace qw {
-int launch_stream2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) { return s2d_launch<double>(s, in_buf, out_buf, k, box); }
+int launch_stream2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) { return s2d_launch<double, false>(s, in_buf, out_buf, k, box); }
 }  // namespace qw

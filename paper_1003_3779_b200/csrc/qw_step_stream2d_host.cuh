@@ -57,10 +57,10 @@ static S2dPlan s2d_plan(const Box &box, long long batch, int VN, int K, long lon
     return best;
 }
 
-template <typename R, int KIND, int K>
+template <typename R, int KIND, int K, bool RBL>
 static int s2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     typedef typename Cx<R>::T V;
-    constexpr int RN = S2dShape<R, K>::RN, HN = 32 * RN, VN = HN - 2 * K, WPC = S2dShape<R, K>::WPC;
+    constexpr int RN = S2dShape<R, K, RBL>::RN, HN = 32 * RN, VN = HN - 2 * K, WPC = S2dShape<R, K, RBL>::WPC;
     const Geom &g = s->g;
     Stream2dArgs<R> a;
     a.in = static_cast<const V *>(state_ptr(s, in_buf));
@@ -75,6 +75,9 @@ static int s2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     for (int i = 0; i < K - 1; ++i) pw *= scale;
     for (int i = 0; i < 32; ++i) a.coin_last[i] = (R)(s->h_coin[i] * pw);
     a.ratio = KIND == COIN_GROVER4 ? (R)((s->h_coin[0] - s->h_coin[2]) / s->h_coin[2]) : (R)0;
+    a.rbl_key0 = (unsigned)(s->rbl_seed & 0xffffffffu); a.rbl_key1 = (unsigned)(s->rbl_seed >> 32);
+    a.rbl_thr = s->rbl_thr;
+    a.t = (unsigned)((unsigned long long)s->t & 0xffffffffu);     // level l of the pipeline = step t + l
     // diamond of the light cone after this launch; on a torus only while the square box has not wrapped
     a.dia_r = -1; a.dia_m = s->centre[0]; a.dia_n = s->centre[1];
     if (s->window_enabled && s->window_valid) {
@@ -91,13 +94,13 @@ static int s2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     a.units = (long long)g.batch * plan.segs * plan.strips;
     const long long need = (a.units + WPC - 1) / WPC;
     const unsigned grid = (unsigned)(need < ctas ? need : ctas);
-    const size_t smem = stream2d_smem_bytes<R, K>();
+    const size_t smem = stream2d_smem_bytes<R, K, RBL>();
     auto go = [&](auto kernel) -> int {
         QW_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         kernel<<<grid, WPC * 32, smem, s->stream>>>(a);
         return QW_OK;
     };
-    int rc = g.boundary == QW_OPEN ? go(step_stream2d_kernel<R, KIND, true, K>) : go(step_stream2d_kernel<R, KIND, false, K>);
+    int rc = g.boundary == QW_OPEN ? go(step_stream2d_kernel<R, KIND, true, K, RBL>) : go(step_stream2d_kernel<R, KIND, false, K, RBL>);
     if (rc) return rc;
     QW_LAUNCH_CHECK(s, "step_stream2d_kernel");
     {   // site-steps actually computed: the valid outputs of the units the kernel's diamond test leaves active
@@ -117,30 +120,33 @@ static int s2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     return QW_OK;
 }
 
-template <typename R, int KIND>
+template <typename R, int KIND, bool RBL>
 static int s2d_launch_kind(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
     switch (k) {
 #ifndef QW_S2D_DEV                    // (tuning builds compile the deep float instances of one coin only)
-        case 2: return s2d_launch_k<R, KIND, 2>(s, in_buf, out_buf, box);
-        case 4: return s2d_launch_k<R, KIND, 4>(s, in_buf, out_buf, box);
-        case 6: return s2d_launch_k<R, KIND, 6>(s, in_buf, out_buf, box);
+        case 2: return s2d_launch_k<R, KIND, 2, RBL>(s, in_buf, out_buf, box);
+        case 4: return s2d_launch_k<R, KIND, 4, RBL>(s, in_buf, out_buf, box);
+        case 6: return s2d_launch_k<R, KIND, 6, RBL>(s, in_buf, out_buf, box);
 #endif
-        case 8: return s2d_launch_k<R, KIND, 8>(s, in_buf, out_buf, box);
-        case 10: return s2d_launch_k<R, KIND, 10>(s, in_buf, out_buf, box);
-        case 12: return s2d_launch_k<R, KIND, 12>(s, in_buf, out_buf, box);
-        default: return fail(QW_EINVAL, "streaming 2D step depth %d is not one of 2, 4, 6, 8, 10, 12", k);
+        case 8: return s2d_launch_k<R, KIND, 8, RBL>(s, in_buf, out_buf, box);
+        default: break;
     }
+    if constexpr (!RBL && sizeof(R) == 4) {      // the deep pipelines: complex64 without link draws (stream2d_max_k)
+        if (k == 10) return s2d_launch_k<R, KIND, 10, RBL>(s, in_buf, out_buf, box);
+        if (k == 12) return s2d_launch_k<R, KIND, 12, RBL>(s, in_buf, out_buf, box);
+    }
+    return fail(QW_EINVAL, "streaming 2D step depth %d has no kernel instance here", k);
 }
 
-template <typename R>
+template <typename R, bool RBL>
 static int s2d_launch(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
     switch (s->coin_kind) {
 #ifndef QW_S2D_DEV
-        case COIN_GROVER4: return s2d_launch_kind<R, COIN_GROVER4>(s, in_buf, out_buf, k, box);
-        case COIN_HXH4:    return s2d_launch_kind<R, COIN_HXH4>(s, in_buf, out_buf, k, box);
+        case COIN_GROVER4: return s2d_launch_kind<R, COIN_GROVER4, RBL>(s, in_buf, out_buf, k, box);
+        case COIN_HXH4:    return s2d_launch_kind<R, COIN_HXH4, RBL>(s, in_buf, out_buf, k, box);
 #endif
-        case COIN_DFT4:    return s2d_launch_kind<R, COIN_DFT4>(s, in_buf, out_buf, k, box);
-        default:           return s2d_launch_kind<R, COIN_GENERAL>(s, in_buf, out_buf, k, box);
+        case COIN_DFT4:    return s2d_launch_kind<R, COIN_DFT4, RBL>(s, in_buf, out_buf, k, box);
+        default:           return s2d_launch_kind<R, COIN_GENERAL, RBL>(s, in_buf, out_buf, k, box);
     }
 }
 

@@ -232,3 +232,49 @@ def test_ensemble_average_over_the_batch(qw, oracle, dev, dtype, dim):
             assert float(np.max(np.abs(host.astype(np.float64) - P[0].astype(np.float64)))) <= tol
         else:                 # the realisations differ, the average is none of them
             assert float(np.max(np.abs(P[0].astype(np.float64) - P[1].astype(np.float64)))) > 1e-6
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.PERIODIC, qi.OPEN])
+def test_rbl_inside_the_streaming_2d_kernel(qw, oracle, dev, dtype, boundary):
+    """Random broken links drawn INSIDE the temporally blocked 2D kernel (eqs. 9-10; reading R27): level l of
+    the row pipeline is step t + l, one generator call per lane, level and row for the four links its two sites own, the
+    bit of the link to the next lane travels by shuffle, a broken link along m swaps phi_2 with the parked phi_1 one
+    cascade later.  Streaming == fused-RBL bit for bit (same link function, same coin arithmetic) and parity with the
+    oracle: several strips and segments, walls, batches (the walk index is part of the counter), every depth, split
+    stepping (the step index carries over), p = 1 (every link broken: nothing moves)."""
+    rng = np.random.default_rng(23)
+    cases = [((70, 96), 13, 0, 1, 0.1), ((64, 64), 12, 2, 3, 0.5), ((201, 130), 16, 4, 1, 0.1), ((97, 200), 18, 6, 2, 0.25),
+             ((130, 72), 16, 8, 1, 0.1), ((48, 40), 8, 4, 1, 1.0)]
+    for extents, steps, k, batch, p in cases:
+        for coin in ("dft", "grover", "random"):
+            c = {"grover": qi.grover4, "dft": qi.dft4}[coin](dtype) if coin != "random" else qi.random_unitary(rng, 4).astype(dtype)
+            sites = extents[0] * extents[1]
+            w = qi.Workload("rbl2d", 2, extents, batch, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c,
+                            state=qi.random_state(43, batch, sites, 4, dtype, normalise_per_walk=True))
+            a = gpu_rbl(qw, w, p, SEED, steps, schedule=qw.QW_SCHED_FUSED)
+            b = gpu_rbl(qw, w, p, SEED, steps, schedule=qw.QW_SCHED_TILED, k=k, split=5 if k else None)
+            assert b[2] == qw.QW_SCHED_TILED
+            assert np.array_equal(a[0], b[0]), (extents, steps, k, coin, p)
+            if sites < 20000 and coin != "grover":
+                close(w, b[0], oracle_rbl(oracle, w, p, SEED, steps))
+    # AUTO takes the streaming kernel; a delta start with the light-cone window; few warps (many units per warp)
+    w = qi.Workload("rbl2d-delta", 2, (121, 122), 1, boundary, np.dtype(dtype), 50, qi.COIN_UNIFORM, qi.grover4(dtype),
+                    delta_site=(60, 61), delta_coin=np.array([0.5, -0.5, -0.5, 0.5], dtype=dtype))
+    a = gpu_rbl(qw, w, 0.2, SEED, w.steps, schedule=qw.QW_SCHED_FUSED, window=False)
+    b = gpu_rbl(qw, w, 0.2, SEED, w.steps, options={qw.QW_OPT_MAX_CTAS: 1})
+    assert b[2] == qw.QW_SCHED_TILED and np.array_equal(a[0], b[0])
+    close(w, b[0], oracle_rbl(oracle, w, 0.2, SEED, w.steps))
+    # rows of odd length: two sites of a lane do not share a generator call -> no streaming instance, AUTO runs fused
+    w = qi.k3(extents=(64, 65), steps=6, coin="dft", dtype=dtype)
+    assert gpu_rbl(qw, w, 0.1, SEED, 6)[2] == qw.QW_SCHED_FUSED
+    h = qw.create_for(w)
+    try:
+        qw.qw_set_random_broken_links(h, 1, 0.1, SEED)
+        qw.qw_set_schedule(h, qw.QW_SCHED_TILED, 0)
+        qw.load_state(h, w)
+        with pytest.raises(qw.QwError) as ei:
+            qw.qw_step(h, 4)
+        assert ei.value.code == qw.QW_EUNSUPPORTED
+    finally:
+        qw.qw_destroy(h)
