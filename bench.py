@@ -616,6 +616,31 @@ def run_gpu(args):
                     "kernels produced (halo / starter recomputation excluded; with the light-cone window only the tiles and warps "
                     "that were not skipped), effective_frac counts the full lattice (BASELINE.json:metric)",
         }
+        if kname == "step_stream2d_kernel" and args.rbl is None and kdepth >= 2:
+            # The streaming 2D kernel reads and writes every amplitude once per launch of k steps, and at its default depth that
+            # is what binds it (ncu: DRAM 83 % of the measured copy peak, FP pipe 52 %; profiles/r02_stream2d.md).  So the
+            # roofline of this kernel is HBM: algorithmic bytes per launch = 2*coin_dim*sizeof(complex) B x the sites it
+            # produced, per launch duration; the instruction-slot figures stay beside it.
+            alu = roofline
+            launch_bytes_per_site = alg_bytes_per_site            # one read + one write of the lattice per launch
+            gbs = rate_touched * launch_bytes_per_site / kdepth / 1e9
+            roofline = {
+                "bound": "hbm", "kernel": kname, "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                "peak_source": "of " + peak_src, "frac_of_nominal_8000": gbs / 8000.0,
+                "effective_frac": rate * launch_bytes_per_site / kdepth / 1e9 / peak,
+                "algorithmic_bytes_per_site_per_launch": launch_bytes_per_site, "steps_per_launch": kdepth,
+                "algorithmic_bytes_per_site_step": launch_bytes_per_site / kdepth,
+                "touched_site_updates_per_bench_step": touched_per_step, "touched_fraction_of_full_lattice": touched_frac,
+                "traffic": stored_traffic(args.workload + "_" + sched_name),
+                "alu_frac": alu["frac"], "alu_effective_frac": alu["effective_frac"], "alu_peak_tflops": alu["peak"],
+                "alu_peak_source": alu["peak_source"], "algorithmic_instr_per_site_step": instr,
+                "algorithmic_flops_per_site_step": flops,
+                "effective_hbm_gbs_vs_single_step": eff_gbs, "single_step_hbm_roofline_x": eff_gbs / peak,
+                "note": "k walk steps per HBM round trip: achieved = algorithmic bytes per launch (2*coin_dim*sizeof(complex) B per "
+                        "site the kernel produced) / launch duration (CUDA events over qw_step, remainder launches and gaps "
+                        "included); alu_frac = FP instructions of the produced site-updates / measured instruction-slot peak; "
+                        "effective_* count the full lattice (BASELINE.json:metric)",
+            }
     if fused is not None:
         fg = fused["site_updates_per_s"] * alg_bytes_per_site / 1e9
         fused.update({"bound": "hbm", "kernel": "step_scatter_kernel (fused coin+shift)", "achieved": fg, "peak": peak,

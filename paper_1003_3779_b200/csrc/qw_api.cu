@@ -476,8 +476,9 @@ int qw_step(qw_sim *s, int64_t n) {
     s->last_sched = sched; s->last_k = 1;
     if (sched == QW_SCHED_TILED) {
         // k-step launches, then the even part of the remainder; an odd last step goes through the fused kernel below
-        // measured optima on B200 (profiles/), both kernels: 8 (complex64) / 6 (complex128); with link draws 6 (registers)
-        const int kmax = s->sched_k > 0 ? s->sched_k : ((s->dtype == QW_C128 || s->rbl) ? 6 : 8);
+        // measured optima on B200 (profiles/), both kernels: 8 (complex64) / 6 (complex128); with link draws (integer
+        // bound, the draws cost registers) 4
+        const int kmax = s->sched_k > 0 ? s->sched_k : (s->rbl ? 4 : (s->dtype == QW_C128 ? 6 : 8));
         s->last_k = kmax;
         while (remaining >= 2) {
             const int kk = (int)(remaining >= kmax ? kmax : remaining / 2 * 2);

@@ -53,6 +53,8 @@ template <int K, bool RBL> struct S2dShape<float, K, RBL> {      // (link draws 
     static constexpr int NS = K <= 8 ? 0 : (K == 10 ? QW_S2D_NS10 : QW_S2D_NS12);
     static constexpr bool WAVE = QW_S2D_WAVE != 0;
 };
+// (complex128 with 64-column strips at k >= 6 — all phi_1 rows in shared memory — was measured and dropped: 1.25e11 against
+// 2.3e11 site-updates/s on the K2 lattice; two 32-byte shared-memory round trips per level and row bind the load/store pipe.)
 template <int K, bool RBL> struct S2dShape<double, K, RBL> {
     static constexpr int RN = (K <= 4) ? 2 : 1, WPC = (K <= (RBL ? 0 : 2)) ? 12 : 8, RING = (K <= 4) ? 4 : 8, PF = RING - 1;
     static constexpr int NS = 0;
