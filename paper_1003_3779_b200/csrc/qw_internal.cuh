@@ -187,6 +187,7 @@ int launch_tiled2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box
 // K-level pipeline of rows in REGISTERS (uniform coin, 2D natural lattice); the 2D AUTO schedule where it applies.
 bool stream2d_eligible(const qw_sim *s);
 int stream2d_max_k(const qw_sim *s);
+bool stream2d_wraps(const qw_sim *s);   // torus: the kernel wraps its input addresses itself (no ghost-ring refresh before the launch)
 int launch_step_stream2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 int launch_stream2d_f32(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);
 int launch_stream2d_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box &box);

@@ -330,8 +330,13 @@ bool stream2d_eligible(const qw_sim *s) {
 }
 int stream2d_max_k(const qw_sim *s) { return (s->dtype == QW_C128 || s->rbl) ? 8 : 12; }
 
+// On a torus the units at the seams wrap their input rows and columns themselves when the rows have even length (a lane's
+// two-column segment then never straddles the seam and stays 16-byte aligned); otherwise the halos come from the refreshed
+// ghost ring.
+bool stream2d_wraps(const qw_sim *s) { return s->g.boundary == QW_PERIODIC && s->g.en % 2 == 0; }
+
 int launch_step_stream2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
-    if (s->g.boundary == QW_PERIODIC) {
+    if (s->g.boundary == QW_PERIODIC && !stream2d_wraps(s)) {
         int rc = launch_ghost_refresh(s, in_buf);
         if (rc) return rc;
     }

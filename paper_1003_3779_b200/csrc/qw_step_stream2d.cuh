@@ -67,6 +67,8 @@ struct Stream2dArgs {
     typename Cx<R>::T *out;       // ... of the output buffer
     long long em, en, pitch, walk_stride, plane_stride;
     long long max_col;            // largest column index a lane may address (row allocation end), a multiple of RN
+    int wrap;                     // torus without the ghost ring: the units at the seams wrap their input rows / columns
+                                  // themselves (rows of even length: lane segments stay whole and aligned)
     int batch;
     int strip0, strips;           // launched range of the global strip grid: strip j owns columns [j*V, (j+1)*V)
     long long row_lo, row_hi;     // launched rows (inclusive), cut into `segs` segments of `seg_len` rows
@@ -413,9 +415,19 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
         constexpr bool WALL = EDGE && OPEN;
         constexpr uint32_t PLB = HN * sizeof(V), SLOTB = 4 * PLB;             // bytes of a plane row / of a ring slot
         const long long col = n0 + lane * RN;
-        const long long lcol = col <= a.max_col ? col : a.max_col;             // lanes beyond the row allocation re-read its end
+        long long lcol = col;
+        long long row0 = a0 - K;                                               // input row a0-K comes first
+        int fseam = -1;                                                        // fetches until the input rows wrap around (torus)
+        if constexpr (EDGE && !OPEN) {
+            if (a.wrap) {                                                      // no ghost ring: wrap rows and columns here
+                if (lcol < 0) lcol += a.en; else if (lcol >= a.en) lcol -= a.en;
+                if (row0 < 0) row0 += a.em;
+                fseam = (int)(a.em - row0);
+            }
+        }
+        if (lcol > a.max_col) lcol = a.max_col;                                // lanes beyond the row allocation re-read its end
         // running byte pointers (plane 0): the next input row to fetch, the next output row to store
-        const char *gp = reinterpret_cast<const char *>(a.in + w * a.walk_stride + (a0 - K) * a.pitch + lcol);
+        const char *gp = reinterpret_cast<const char *>(a.in + w * a.walk_stride + row0 * a.pitch + lcol);
         char *op = reinterpret_cast<char *>(a.out + w * a.walk_stride + a0 * a.pitch + col);
         const long long planeb = a.plane_stride * (long long)sizeof(V);
         const long long rowb = a.pitch * (long long)sizeof(V);
@@ -454,6 +466,7 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
                     g += planeb;
                 }
                 gp += rowb;
+                if constexpr (EDGE && !OPEN) { if (--fseam == 0) gp -= a.em * rowb; }
             }
             --fleft;
             fslot = (fslot + SLOTB) & (RING * SLOTB - 1);
@@ -541,6 +554,7 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
             if (dm + dn > a.dia_r) continue;
         }
         bool edge = n0 + HN >= a.en;               // the strip holds the right end of the rows
+        if constexpr (!OPEN) edge = edge || (a.wrap && (a0 - K < 0 || b0 + K + 1 > a.em || n0 < 0));   // ... or a seam of the torus
         if constexpr (OPEN) edge = edge || (a0 - K <= 0) || (b0 + K >= a.em) || (n0 <= 0);
         if (edge) run(std::true_type{}, w, a0, b0, n0);
         else run(std::false_type{}, w, a0, b0, n0);

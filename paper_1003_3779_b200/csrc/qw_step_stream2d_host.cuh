@@ -67,6 +67,7 @@ static int s2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     a.out = static_cast<V *>(state_ptr(s, out_buf));
     a.em = g.em; a.en = g.en; a.pitch = g.pitch; a.walk_stride = g.walk_stride; a.plane_stride = g.plane_stride;
     a.max_col = (g.pitch - g.ghost - RN) / RN * RN;
+    a.wrap = stream2d_wraps(s) ? 1 : 0;
     a.batch = (int)g.batch;
     for (int i = 0; i < 32; ++i) a.coin[i] = (R)s->h_coin[i];
     // deferred scale (named coins only; their scale is a power of two, so every product below is exact)
