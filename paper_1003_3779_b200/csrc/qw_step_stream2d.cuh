@@ -17,13 +17,25 @@
 // of a strip travels one column per level, so the K outermost columns on each side are a halo (valid = HN - 2K).
 // A segment of rows [a, b) is fed rows a-K .. b+K-1 (the pipeline fills and drains over 2K rows).
 //
-// Memory: each lane copies its own 16-byte pieces of the next input rows into a per-warp ring in shared memory with
-// cp.async (several rows ahead) and reads them back itself, so there is no cross-lane dependency; output rows go from
-// registers to global memory as 16-byte stores.  Halos (rows and columns) come from the ghost ring of the state
-// buffers (periodic: refreshed before each launch).
+// The coin runs in two stages (front / back butterfly, coin_front / coin_back below) so that a level's parked registers
+// are read for the last time BEFORE the level below writes its results into them: no register copies, fixed register
+// roles across the back edge of the row loop (which always runs two cascades per trip).
 //
-// Walls (open lattice = broken outward links, PAPER.md:94-101 with RBL = 0): the outgoing component stays on its site
-// with the opposite coin (3 - c).  Only the units that can see a wall run the instance with the wall code.
+// Memory: each lane copies its own 16-byte pieces of the next input rows into a per-warp ring in shared memory with
+// cp.async (several rows ahead) and reads them back itself, so there is no cross-lane dependency; the row after the
+// current one is already in registers; output rows go from registers to global memory as 16-byte stores.
+// Work units = (walk, segment of rows, strip), strips fastest, round-robin over the warps of the persistent grid; units
+// outside the light-cone diamond are skipped.
+//
+// Halos / walls: open lattice = broken outward links (PAPER.md:94-101 with RBL = 0): the outgoing component stays on
+// its site with the opposite coin (3 - c); what lies outside the lattice is a don't-care.  Torus: the units at the seams
+// wrap their input rows and columns themselves when the rows have even length (Stream2dArgs::wrap), else the halos come
+// from the ghost ring of the state buffers (refreshed before the launch).  Only EDGE units (walls, seams, a lane segment
+// cut by the end of the rows) run the instance with that code and with element-wise stores.
+//
+// Random broken links (RBL instances; eqs. 9-10, R27): level l = step t + l; one Philox call per
+// lane, level and row for the four links its two sites own — see level_step.
+// Deep pipelines (k = 10, 12) park the phi_1 rows of their first levels in shared memory (S2dShape::NS).
 #pragma once
 
 #include <type_traits>
@@ -88,9 +100,6 @@ struct Stream2dArgs {
 namespace s2d {
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void cp_async16(void *dst, const void *src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
 __device__ __forceinline__ void cp_async16_s(uint32_t dst, const void *src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
