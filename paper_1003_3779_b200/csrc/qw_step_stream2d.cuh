@@ -475,7 +475,7 @@ step_stream2d_kernel(const Stream2dArgs<R> a) {
                     g += planeb;
                 }
                 gp += rowb;
-                if constexpr (EDGE && !OPEN) { if (--fseam == 0) gp -= a.em * rowb; }
+                if constexpr (EDGE && !OPEN) { if (--fseam == 0) { gp -= a.em * rowb; fseam = (int)a.em; } }   // (a unit may cross both seams)
             }
             --fleft;
             fslot = (fslot + SLOTB) & (RING * SLOTB - 1);

@@ -434,7 +434,9 @@ def test_streaming_2d_kernel_depths_chains_and_edges(qw, oracle, dev, dtype, bou
     rng = np.random.default_rng(17)
     deep = (10, 12) if dtype == np.complex64 else (8, 6)
     cases = [((211, 97), 27, deep[0], 1, 0), ((64, 49), 24, deep[1], 2, 1), ((301, 145), 20, 8, 1, 2),
-             ((73, 200), 31, 4, 3, 3), ((1000, 129), 16, 0, 1, 0)]
+             ((73, 200), 31, 4, 3, 3), ((1000, 129), 16, 0, 1, 0),
+             # one unit over all rows: on the torus its input crosses the seam twice (rows -k .. em+k-1)
+             ((40, 64), 24, 12 if dtype == np.complex64 else 8, 2, 1)]
     for extents, steps, k, batch, ctas in cases:
         for coin in ("dft", "grover", "random"):
             c = {"grover": qi.grover4, "dft": qi.dft4}[coin](dtype) if coin != "random" else qi.random_unitary(rng, 4).astype(dtype)
