@@ -63,7 +63,8 @@ template <typename R, int K, bool RBL = false> struct S2dShape;
 template <int K, bool RBL> struct S2dShape<float, K, RBL> {      // (link draws cost ~25 registers: 8 warps from k = 4 on)
     static constexpr int RN = 2, WPC = (K <= (RBL ? 2 : 4)) ? 12 : 8, RING = 8, PF = 6;
     static constexpr int NS = K <= 8 ? 0 : (K == 10 ? QW_S2D_NS10 : QW_S2D_NS12);
-    static constexpr bool WAVE = QW_S2D_WAVE != 0;
+    // two rows per trip as a wavefront (cascade2): the default depth only (+1.5 % on K3; it doubles the compile time of an instance)
+    static constexpr bool WAVE = QW_S2D_WAVE != 0 || (K == 8 && !RBL);
 };
 // (complex128 with 64-column strips at k >= 6 — all phi_1 rows in shared memory — was measured and dropped: 1.25e11 against
 // 2.3e11 site-updates/s on the K2 lattice; two 32-byte shared-memory round trips per level and row bind the load/store pipe.)
