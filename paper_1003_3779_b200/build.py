@@ -46,6 +46,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     sources = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
     headers = sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + sorted(glob.glob(os.path.join(INCLUDE, "*.h")))
     headers.append(os.path.abspath(__file__))
+    if not force and not _stale(LIB, sources + headers):
+        return LIB                                 # the library is newer than every source: nothing to do (objects may be absent)
     jobs = []
     objs = []
     for src in sources:
