@@ -193,6 +193,17 @@ int qw_probabilities_mean(const qw_sim *s, void *out);
  * mean and (population) variance are divided by the computed norm (eq. 4 fixes norm = 1). */
 int qw_moments(const qw_sim *s, double *out);
 
+/* qw_moments for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): same kernels, same result layout, but the block partial sums live in a static device array of the library
+ * (512 KiB, held by every GPU that loads the library until exit) instead of a lazily grown cudaMalloc buffer, and `out`
+ * must be DEVICE memory (batch * 3 doubles in 1D, batch * 6 in 2D); the call performs no cudaMalloc / cudaFree and is
+ * asynchronous on the handle's stream.  Limit: batch <= 8192 walks, else QW_EUNSUPPORTED; QW_EINVAL for a host `out`.
+ * The blocks per walk are capped by the array, so the summation order — and the last bits of the result — can differ
+ * from qw_moments (same tolerance against the definition).  All calls on a device SHARE the array: calls in one stream are
+ * safe back to back (each call rewrites every entry it reads), calls that overlap on the GPU (other streams, other
+ * handles) race. */
+int qw_moments_static(const qw_sim *s, double *out);
+
 /* Force a schedule (QW_SCHED_*); k = temporal block depth for QW_SCHED_BLOCKED / QW_SCHED_TILED
  * (0 = library default; QW_SCHED_TILED accepts the even depths listed at QW_SCHED_TILED, else QW_EINVAL).
  * QW_EUNSUPPORTED if the handle's configuration has no such kernel. */

@@ -29,7 +29,7 @@ QW_OPT_MAX_CTAS, QW_OPT_BLOCKED1D_KERNEL, QW_OPT_TILED2D_KERNEL = 0, 1, 2
 SYMBOLS = (
     "qw_create", "qw_create_batch", "qw_destroy", "qw_set_stream", "qw_set_lattice", "qw_set_coin",
     "qw_set_site_phases", "qw_set_broken_links", "qw_set_random_broken_links", "qw_set_state", "qw_set_state_delta", "qw_get_state",
-    "qw_step", "qw_step_inverse", "qw_probabilities", "qw_probabilities_mean", "qw_moments", "qw_set_schedule", "qw_set_window",
+    "qw_step", "qw_step_inverse", "qw_probabilities", "qw_probabilities_mean", "qw_moments", "qw_moments_static", "qw_set_schedule", "qw_set_window",
     "qw_set_option", "qw_get_info", "qw_measure_alu_peak", "qw_synchronize", "qw_last_error",
 )
 
@@ -73,6 +73,7 @@ def load(path: Optional[str] = None) -> ctypes.CDLL:
         "qw_probabilities": [vp, vp],
         "qw_probabilities_mean": [vp, vp],
         "qw_moments": [vp, vp],
+        "qw_moments_static": [vp, vp],
         "qw_set_schedule": [vp, ci, ci],
         "qw_set_window": [vp, ci],
         "qw_set_option": [vp, ci, i64],
@@ -191,6 +192,11 @@ def qw_probabilities_mean(h, out) -> None:
 
 def qw_moments(h, out) -> None:
     _check(load().qw_moments(h, _ptr(out)))
+
+
+def qw_moments_static(h, out) -> None:
+    """qw_moments without any allocation: `out` must be a device tensor (include/qw.h)."""
+    _check(load().qw_moments_static(h, _ptr(out)))
 
 
 def qw_set_schedule(h, schedule, k=0) -> None:

@@ -628,6 +628,17 @@ int qw_moments(const qw_sim *cs, double *out) {
     return QW_OK;
 }
 
+int qw_moments_static(const qw_sim *cs, double *out) {
+    clear_error();
+    qw_sim *s = const_cast<qw_sim *>(cs);
+    if (!s) return fail(QW_EINVAL, "handle is NULL");
+    QW_ON_DEVICE(s);
+    if (!out) return fail(QW_EINVAL, "out is NULL");
+    if (!s->has_state) return fail(QW_ESTATE, "no state has been set");
+    if (!is_device_ptr(out)) return fail(QW_EINVAL, "qw_moments_static writes to DEVICE memory only (a host buffer would need a staging allocation)");
+    return launch_moments_static(s, state_ptr(s, s->cur), out);
+}
+
 int qw_set_schedule(qw_sim *s, int schedule, int k) {
     clear_error();
     if (!s) return fail(QW_EINVAL, "handle is NULL");

@@ -198,5 +198,6 @@ int launch_stream2d_rbl_f64(qw_sim *s, int in_buf, int out_buf, int k, const Box
 int launch_probabilities(qw_sim *s, const void *state, void *out_dev);
 int launch_probabilities_mean(qw_sim *s, const void *state, void *out_dev);   // [sites], mean over the batch
 int launch_moments(qw_sim *s, const void *state, double *out_dev);
+int launch_moments_static(qw_sim *s, const void *state, double *out_dev);   // partials in a static device array: no allocation
 
 }  // namespace qw

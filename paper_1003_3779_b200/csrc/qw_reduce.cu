@@ -315,4 +315,65 @@ int launch_moments(qw_sim *s, const void *state, double *out) {
     return QW_OK;
 }
 
+// ---- moments without any allocation (qw_moments_static) --------------------------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+// the same two kernels as launch_moments, with the block partials in a file-scope device array of a fixed, modest size
+// instead of the handle's lazily grown cudaMalloc buffer.  Every GPU that loads the library holds the array
+// (QW_STATIC_PARTIAL_BLOCKS * NPART doubles = 512 KiB) until exit.  ALL calls on a device share it: every call overwrites
+// all NPART entries of every block it uses before the second kernel reads them (nothing has to start at zero, nothing is
+// accumulated across calls), so calls in ONE stream are safe one after the other, while calls that overlap on the GPU
+// (different streams or handles at the same time) race.
+constexpr long long QW_STATIC_PARTIAL_BLOCKS = 8192;
+static __device__ __align__(256) double qw_static_partials[QW_STATIC_PARTIAL_BLOCKS * NPART];
+
+// In host code the array's name is a host-side stand-in, not a device address: its device address is looked up once per
+// device, with that device current, and that pointer is what the kernels get.
+static double *static_partials_ptr(int device) {
+    constexpr int MAXDEV = 64;
+    static double *ptr[MAXDEV] = {};
+    if (device < 0 || device >= MAXDEV) return nullptr;
+    if (!ptr[device]) {
+        double *p = nullptr;
+        if (cudaGetSymbolAddress((void **)&p, qw_static_partials) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        ptr[device] = p;
+    }
+    return ptr[device];
+}
+
+template <typename R, int CD>
+static void launch_mom_static_t(qw_sim *s, const void *state, double *partials, unsigned grid, int bpw, long long ipb, int cpr) {
+    const Geom &g = s->g;
+    moments_partial_kernel<R, CD><<<grid, RED_BLOCK, 0, s->stream>>>(
+        static_cast<const typename Cx<R>::T *>(state), partials, g.em, g.en, g.pitch, g.walk_stride, g.plane_stride, bpw, ipb, cpr);
+}
+
+// out: DEVICE pointer.  The caller (qw_moments_static) has made s->device the current device.
+int launch_moments_static(qw_sim *s, const void *state, double *out) {
+    const Geom &g = s->g;
+    if (g.batch > QW_STATIC_PARTIAL_BLOCKS)
+        return fail(QW_EUNSUPPORTED, "qw_moments_static holds the partial sums of at most %lld blocks: batch %lld is too large "
+                                     "(use qw_moments, which allocates)", QW_STATIC_PARTIAL_BLOCKS, g.batch);
+    const int vec = s->dtype == QW_C128 ? RedVec<double>::value : RedVec<float>::value;
+    const int cpr = (int)((g.en + (long long)RED_BLOCK * vec - 1) / ((long long)RED_BLOCK * vec));
+    const long long items = g.em * cpr;
+    // as launch_moments, with the blocks per walk capped by what the static array holds
+    long long bpw = (long long)s->sm_count * 32 / g.batch;
+    if (bpw > QW_STATIC_PARTIAL_BLOCKS / g.batch) bpw = QW_STATIC_PARTIAL_BLOCKS / g.batch;
+    if (bpw < 1) bpw = 1;
+    if (bpw > items) bpw = items;
+    const long long ipb = (items + bpw - 1) / bpw;
+    bpw = (items + ipb - 1) / ipb;
+    const long long blocks = bpw * g.batch;
+    if (blocks > QW_STATIC_PARTIAL_BLOCKS) return fail(QW_EUNSUPPORTED, "qw_moments_static: %lld blocks exceed the static scratch", blocks);
+    double *partials = static_partials_ptr(s->device);
+    if (!partials) return fail(QW_ECUDA, "cudaGetSymbolAddress(qw_static_partials) failed on device %d", s->device);
+    if (s->dtype == QW_C128) { if (g.cdim == 2) launch_mom_static_t<double, 2>(s, state, partials, (unsigned)blocks, (int)bpw, ipb, cpr); else launch_mom_static_t<double, 4>(s, state, partials, (unsigned)blocks, (int)bpw, ipb, cpr); }
+    else                     { if (g.cdim == 2) launch_mom_static_t<float, 2>(s, state, partials, (unsigned)blocks, (int)bpw, ipb, cpr);  else launch_mom_static_t<float, 4>(s, state, partials, (unsigned)blocks, (int)bpw, ipb, cpr); }
+    QW_LAUNCH_CHECK(s, "moments_partial_kernel");
+    const int warps = 4;
+    moments_final_kernel<<<(unsigned)((g.batch + warps - 1) / warps), warps * 32, 0, s->stream>>>(partials, out, g.batch, (int)bpw, g.dim);
+    QW_LAUNCH_CHECK(s, "moments_final_kernel");
+    return QW_OK;
+}
+
 }  // namespace qw
