@@ -76,7 +76,7 @@ enum {
     QW_SCHED_TILED = 5     /* 2D temporally blocked with the state of k steps held in REGISTERS; honours the
                               light-cone window.  Natural lattice, any boundary: every warp streams down a strip
                               of columns with a k-level pipeline of rows in its registers (no halo along m, no
-                              barriers; k even, <= 12 for complex64, <= 8 for complex128), or — QW_OPT_TILED2D_KERNEL
+                              barriers; k even, <= 10 for complex64, <= 8 for complex128, <= 6 with random broken links), or — QW_OPT_TILED2D_KERNEL
                               — tiles held by persistent CTAs with TMA prefetch (k in {2, 4, 6, 8}).  Diagonal
                               lattice (tiles only): torus, or open lattice after qw_set_state_delta (the fused
                               kernel takes over when the cone reaches a wall)                                  */

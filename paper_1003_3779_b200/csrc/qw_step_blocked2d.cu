@@ -321,14 +321,14 @@ int launch_step_tiled2d(qw_sim *s, int in_buf, int out_buf, int k, const Box &bo
 
 // Streaming schedule (qw_step_stream2d.cuh): natural lattice, uniform coin; same ghost ring as the tiles.
 // Random broken links redrawn every step are drawn inside the kernel when the rows have even length (two sites of a
-// lane share one generator call); depth <= 8 then.
+// lane share one generator call); depth <= 6 then.
 bool stream2d_eligible(const qw_sim *s) {
     const Geom &g = s->g;
     return g.dim == 2 && g.lattice == QW_NATURAL && s->coin_mode == QW_COIN_UNIFORM && !s->d_phases && !s->d_broken &&
            (!s->rbl || g.en % 2 == 0) && g.em >= 2 * QW_GHOST_2D && g.en >= 2 * QW_GHOST_2D && g.batch <= 16383 &&
            g.walk_stride * 4 * g.batch < (1LL << 40);
 }
-int stream2d_max_k(const qw_sim *s) { return (s->dtype == QW_C128 || s->rbl) ? 8 : 12; }
+int stream2d_max_k(const qw_sim *s) { return s->rbl ? 6 : (s->dtype == QW_C128 ? 8 : 10); }
 
 // On a torus the units at the seams wrap their input rows and columns themselves when the rows have even length (a lane's
 // two-column segment then never straddles the seam and stays 16-byte aligned); otherwise the halos come from the refreshed

@@ -35,7 +35,7 @@
 //
 // Random broken links (RBL instances; eqs. 9-10, R27): level l = step t + l; one Philox call per
 // lane, level and row for the four links its two sites own — see level_step.
-// Deep pipelines (k = 10, 12) park the phi_1 rows of their first levels in shared memory (S2dShape::NS).
+// The deep pipeline (k = 10) parks the phi_1 rows of its first levels in shared memory (S2dShape::NS).
 #pragma once
 
 #include <type_traits>
@@ -58,11 +58,10 @@ template <typename R, int K, bool RBL = false> struct S2dShape;
 // load and store per level and row): what lets the deep pipelines fit the register file.
 #ifndef QW_S2D_NS10
 #define QW_S2D_NS10 5
-#define QW_S2D_NS12 8
 #endif
 template <int K, bool RBL> struct S2dShape<float, K, RBL> {      // (link draws cost ~25 registers: 8 warps from k = 4 on)
     static constexpr int RN = 2, WPC = (K <= (RBL ? 2 : 4)) ? 12 : 8, RING = 8, PF = 6;
-    static constexpr int NS = K <= 8 ? 0 : (K == 10 ? QW_S2D_NS10 : QW_S2D_NS12);
+    static constexpr int NS = K <= 8 ? 0 : QW_S2D_NS10;
     // two rows per trip as a wavefront (cascade2): the default depth only (+1.5 % on K3; it doubles the compile time of an instance)
     static constexpr bool WAVE = QW_S2D_WAVE != 0 || (K == 8 && !RBL);
 };

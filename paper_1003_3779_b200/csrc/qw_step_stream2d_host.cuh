@@ -121,23 +121,29 @@ static int s2d_launch_k(qw_sim *s, int in_buf, int out_buf, const Box &box) {
     return QW_OK;
 }
 
+// Instances: depths 2 .. 8 (2 .. 6 with link draws, which spill beyond), + 10 for complex64 without link draws.  (k = 12 was
+// built and measured — never faster than k = 8 or 10, profiles/r02_stream2d.md — and dropped for its compile time.)
+// Not static: the coins of one dtype are spread over two translation units (QW_S2D_EXTERN / QW_S2D_DEFINE below).
 template <typename R, int KIND, bool RBL>
-static int s2d_launch_kind(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
+int s2d_launch_kind(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {
     switch (k) {
 #ifndef QW_S2D_DEV                    // (tuning builds compile the deep float instances of one coin only)
         case 2: return s2d_launch_k<R, KIND, 2, RBL>(s, in_buf, out_buf, box);
         case 4: return s2d_launch_k<R, KIND, 4, RBL>(s, in_buf, out_buf, box);
         case 6: return s2d_launch_k<R, KIND, 6, RBL>(s, in_buf, out_buf, box);
 #endif
-        case 8: return s2d_launch_k<R, KIND, 8, RBL>(s, in_buf, out_buf, box);
         default: break;
     }
-    if constexpr (!RBL && sizeof(R) == 4) {      // the deep pipelines: complex64 without link draws (stream2d_max_k)
-        if (k == 10) return s2d_launch_k<R, KIND, 10, RBL>(s, in_buf, out_buf, box);
-        if (k == 12) return s2d_launch_k<R, KIND, 12, RBL>(s, in_buf, out_buf, box);
+    if constexpr (!RBL) {
+        if (k == 8) return s2d_launch_k<R, KIND, 8, RBL>(s, in_buf, out_buf, box);
+        if constexpr (sizeof(R) == 4) {          // the deep pipeline: complex64 without link draws (stream2d_max_k)
+            if (k == 10) return s2d_launch_k<R, KIND, 10, RBL>(s, in_buf, out_buf, box);
+        }
     }
     return fail(QW_EINVAL, "streaming 2D step depth %d has no kernel instance here", k);
 }
+#define QW_S2D_EXTERN(R, KIND, RBL) extern template int s2d_launch_kind<R, KIND, RBL>(qw_sim *, int, int, int, const Box &);
+#define QW_S2D_DEFINE(R, KIND, RBL) template int s2d_launch_kind<R, KIND, RBL>(qw_sim *, int, int, int, const Box &);
 
 template <typename R, bool RBL>
 static int s2d_launch(qw_sim *s, int in_buf, int out_buf, int k, const Box &box) {

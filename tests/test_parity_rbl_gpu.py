@@ -245,7 +245,7 @@ def test_rbl_inside_the_streaming_2d_kernel(qw, oracle, dev, dtype, boundary):
     stepping (the step index carries over), p = 1 (every link broken: nothing moves)."""
     rng = np.random.default_rng(23)
     cases = [((70, 96), 13, 0, 1, 0.1), ((64, 64), 12, 2, 3, 0.5), ((201, 130), 16, 4, 1, 0.1), ((97, 200), 18, 6, 2, 0.25),
-             ((130, 72), 16, 8, 1, 0.1), ((48, 40), 8, 4, 1, 1.0)]
+             ((130, 72), 16, 6, 1, 0.1), ((48, 40), 8, 4, 1, 1.0)]
     for extents, steps, k, batch, p in cases:
         for coin in ("dft", "grover", "random"):
             c = {"grover": qi.grover4, "dft": qi.dft4}[coin](dtype) if coin != "random" else qi.random_unitary(rng, 4).astype(dtype)
