@@ -23,6 +23,19 @@ static inline bool s2d_unit_active(long long a0, long long b0, long long n_lo, l
     return dm + dn <= dr;
 }
 
+// number of strips of the launched range [strip0, strip0 + strips) that meet the diamond in the segment of rows [a0, b0): they
+// form one interval (the kernel enumerates it with the same formula)
+static inline long long s2d_row_count(long long a0, long long b0, int strip0, int strips, int VN, long long dm0, long long dn0, long long dr) {
+    if (a0 >= b0) return 0;
+    const long long dm = dm0 < a0 ? a0 - dm0 : (dm0 > b0 - 1 ? dm0 - (b0 - 1) : 0);
+    const long long rem = dr - dm;
+    if (rem < 0) return 0;
+    long long lo = (dn0 - rem) / VN, hi = (dn0 + rem) / VN;
+    if (lo < strip0) lo = strip0;
+    if (hi > strip0 + strips - 1) hi = strip0 + strips - 1;
+    return hi >= lo ? hi - lo + 1 : 0;
+}
+
 // Segments per strip: every segment costs seg_len + 2K row cascades (the pipeline fills and drains), the launch takes
 // ceil(active units / warps) rounds of them.  Candidates: the segment counts that fill 1 .. 8 rounds of the grid.
 static S2dPlan s2d_plan(const Box &box, long long batch, int VN, int K, long long warps, long long dm0, long long dn0, long long dr) {
@@ -53,6 +66,26 @@ static S2dPlan s2d_plan(const Box &box, long long batch, int VN, int K, long lon
         const double cost = (double)((active + warps - 1) / warps) * (double)(len + 2 * K + 2);
         if (best.cost < 0 || cost < best.cost) { best.segs = (int)segs; best.seg_len = len; best.cost = cost; }
         if (shortest) break;                                      // the segments cannot get any shorter
+    }
+    // With a diamond the active units are dealt round-robin (the kernel enumerates them), so the launch takes
+    // ceil(active / warps) rounds: every segment count is a candidate (the active count of a segment row is closed-form).
+    if (dr >= 0) {
+        const long long max_segs = rows / (2LL * K) > 0 ? rows / (2LL * K) : 1;
+        long long prev_len = -1;
+        for (long long sg_n = 1; sg_n <= max_segs; ++sg_n) {
+            const long long len = (rows + sg_n - 1) / sg_n;
+            if (len == prev_len) continue;
+            prev_len = len;
+            const long long segs = (rows + len - 1) / len;
+            long long active = 0;
+            for (long long sg = 0; sg < segs; ++sg) {
+                const long long a0 = box.m_lo + sg * len, b0 = a0 + len <= box.m_hi + 1 ? a0 + len : box.m_hi + 1;
+                active += s2d_row_count(a0, b0, best.strip0, best.strips, VN, dm0, dn0, dr);
+            }
+            active *= batch;
+            const double cost = (double)((active + warps - 1) / warps) * (double)(len + 2 * K + 2);
+            if (cost < best.cost) { best.segs = (int)segs; best.seg_len = len; best.cost = cost; }
+        }
     }
     return best;
 }
