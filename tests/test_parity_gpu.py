@@ -622,6 +622,39 @@ def test_light_cone_diamond_of_the_tiled_kernel(qw, oracle, dev, dtype, coin, ke
 
 
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("boundary", [qi.OPEN, qi.PERIODIC])
+def test_streaming_2d_kernel_enumerates_the_active_units_of_the_diamond(qw, oracle, dev, dtype, boundary):
+    """With the light-cone diamond the streaming kernel deals only the ACTIVE units (per segment row the strips that meet the
+    diamond: one interval in closed form) to its warps.  A batch (the scan runs over walks x segments), off-centre starts cut
+    by the walls / close to the seams, many and few warps (QW_OPT_MAX_CTAS: every warp takes many units / every warp at most
+    one), steps split over calls so that cones of many radii are launched: window on == window off (fused) bit for bit, and
+    parity with the oracle."""
+    c = qi.grover4(dtype)
+    dc = np.array([0.5, -0.5, -0.5, 0.5], dtype=dtype)
+    for ext, site, steps, batch, ctas in (((230, 310), (100, 150), 96, 3, 0), ((230, 310), (12, 290), 70, 2, 1),
+                                          ((401, 130), (200, 64), 120, 1, 2)):
+        w = qi.Workload("dia-batch", 2, ext, batch, boundary, np.dtype(dtype), steps, qi.COIN_UNIFORM, c, delta_site=site, delta_coin=dc)
+        off = gpu_run(qw, w, schedule=qw.QW_SCHED_FUSED, window=False)
+        h = qw.create_for(w)
+        try:
+            qw.qw_set_option(h, qw.QW_OPT_TILED2D_KERNEL, 2)
+            qw.qw_set_option(h, qw.QW_OPT_MAX_CTAS, ctas)
+            qw.qw_set_schedule(h, qw.QW_SCHED_TILED, 0)
+            qw.load_state(h, w)
+            done = 0
+            for n in (6, 20, 2, steps - 28):
+                qw.qw_step(h, n); done += n
+            assert done == steps and qw.qw_get_info(h, qw.QW_INFO_WINDOW) in (0, 1)
+            got = np.empty((batch, w.sites, 4), dtype=w.dtype)
+            qw.qw_get_state(h, got)
+        finally:
+            qw.qw_destroy(h)
+        assert np.array_equal(got, off[0]), (ext, site, boundary)
+        if batch == 1:
+            check_parity(w, gpu_run(qw, w, schedule=qw.QW_SCHED_TILED, options={qw.QW_OPT_TILED2D_KERNEL: 2}), oracle_run(oracle, w))
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 def test_coin_family_fast_paths(qw, oracle, dev, dtype):
     """PAPER.md:35-38 eq. 1 "collections C = (C_v)": per-walk matrices and / or per-site phases on lattices too long for
     the resident kernel.  The vectorised fused kernel (FAM instance) and, on rings, the chained blocked kernel (phases
