@@ -641,6 +641,10 @@ def run_gpu(args):
                         "included); alu_frac = FP instructions of the produced site-updates / measured instruction-slot peak; "
                         "effective_* count the full lattice (BASELINE.json:metric)",
             }
+    if args.rbl is not None and roofline.get("bound") == "alu":
+        roofline["note"] += ("; with --rbl the temporally blocked kernels are bound by the INTEGER instructions of the in-kernel link "
+                             "draws (one Philox4x32-10 call per four links, ~64 integer instructions), which frac does not count: "
+                             "profiles/r02_stream2d.md section 3, r02_chain1d.md")
     if fused is not None:
         fg = fused["site_updates_per_s"] * alg_bytes_per_site / 1e9
         fused.update({"bound": "hbm", "kernel": "step_scatter_kernel (fused coin+shift)", "achieved": fg, "peak": peak,
